@@ -1,0 +1,208 @@
+/* pairings.h — C ABI of libpairings_b200.so
+ *
+ * Exact counting of Skolem pairings S(n) and Langford pairings L(n) by Godfrey's algebraic
+ * sign-vector sum ("Counting Skolem Sequences", arxiv 1507.00315, §2.1, Lemma 2.1,
+ * PAPER.md:166-168):
+ *
+ *      D(n) = 2^{-2n} * sum_{x in {+1,-1}^{2n}} (prod_i x_i) * prod_{k=1}^{n} P_k(x),
+ *      P_k(x) = sum_{i=1}^{2n-d_k} x_i x_{i+d_k},   d_k = k (Skolem)  or  k+1 (Langford).
+ *
+ * D(n) counts reflected sequences as distinct (A004075 / A176127); the paper's headline numbers
+ * S(n), L(n) identify reflections and are D(n)/2 for n > 1.  Lemma 2.2
+ * lets x_1 be fixed to +1:  H = sum_{x: x_1=+1} term(x) = 2^{2n-1} D(n).
+ *
+ * The path:  host partitioner (pairings_partition / journal)  ->
+ * count_pairings (one sm_100a kernel per chunk range: Gray-code walk, residues modulo
+ * word-size primes)  ->  pairings_sum_rows  ->  pairings_reconstruct (CRT).
+ *
+ * Conventions common to all entry points
+ *   - return 0 (PAIRINGS_OK) on success, a negative PAIRINGS_E* code on error; never throw, abort or print.
+ *   - the caller owns every buffer; "HOST" / "DEVICE" says where a pointer must live.
+ *   - thread-safe; no global mutable state.  There is no CPU fallback: without a CUDA device the
+ *     compute entry points return PAIRINGS_ECUDA.
+ *
+ * Index <-> position contract (binding; it makes per-chunk rows and journals portable):
+ *   N = 2n positions, x_1 = +1, B = 2n-1 index bits.  Index v in [0, 2^B); bit b of v (b = 0..B-1)
+ *   is position N-b; bit = 1 means x = -1.  With C = chunk_bits, chunk c in [0, 2^C) is the set of
+ *   all v with (v >> (B-C)) == c, i.e. x_2..x_{C+1} fixed, most significant chunk bit <-> x_2.
+ *   Row value = T(c) mod p_i with T(c) = sum_{v in chunk c} term(x(v)) as an exact signed integer
+ *   and the mathematical (non-negative) residue in [0, p_i).
+ */
+#ifndef PAIRINGS_B200_H
+#define PAIRINGS_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { PAIRINGS_SKOLEM = 0, PAIRINGS_LANGFORD = 1 };
+
+enum {
+    PAIRINGS_OK = 0,
+    PAIRINGS_EINVAL_KIND = -1,    /* kind is not PAIRINGS_SKOLEM / PAIRINGS_LANGFORD */
+    PAIRINGS_EINVAL_N = -2,       /* n outside [2, 32] */
+    PAIRINGS_EINVAL_CHUNK = -3,   /* chunk_bits outside [0, 2n-1] or range outside [0, 2^chunk_bits] or begin > end */
+    PAIRINGS_EINVAL_MODULUS = -4, /* a modulus is even, outside (2^30, 2^31), duplicated, or n_moduli outside [1, 16] */
+    PAIRINGS_ENULL = -5,          /* a required pointer is NULL */
+    PAIRINGS_ECUDA = -6,          /* CUDA runtime error (no device, launch failure, allocation failure) */
+    PAIRINGS_ECHECK = -7,         /* CRT value disagrees with the redundant check prime */
+    PAIRINGS_EINEXACT = -8,       /* H not divisible by 2^{2n-1}, or D odd (reading A16: never truncate) */
+    PAIRINGS_ERANGE = -9,         /* product of the CRT moduli too small for the bound, or output buffer too small */
+    PAIRINGS_EINVAL_OPTS = -10,   /* launch options not satisfiable for this (kind, n, chunk_bits) */
+    PAIRINGS_EJOURNAL = -11       /* journal file unreadable, or written for other parameters */
+};
+
+#define PAIRINGS_MAX_MODULI 16
+
+/* ------------------------------------------------------------------------------------------------
+ * count_pairings — §8(a) rows a2..a6: the Gray-code / residue kernel.
+ *
+ * Enqueues on `stream` the evaluation of chunks [chunk_begin, chunk_end) of the 2^chunk_bits chunks
+ * and writes, for each chunk c and modulus i, T(c) mod moduli[i] to
+ *      out_residues[(c - chunk_begin) * n_moduli + i]          (row-major, uint32, values in [0, p_i)).
+ * This (chunk_end-chunk_begin) x n_moduli matrix is the only HBM traffic of the path.
+ *
+ *   kind, n        PAIRINGS_SKOLEM / PAIRINGS_LANGFORD, 2 <= n <= 32.  Values of n for which no
+ *                  pairing exists are legal and yield rows that sum to zero.
+ *   chunk_bits     C, 0 <= C <= 2n-1.
+ *   moduli         HOST pointer, n_moduli distinct odd values in (2^30, 2^31), read at call time
+ *                  (primality is the caller's responsibility; pairings_default_moduli supplies primes).
+ *   out_residues   DEVICE pointer, (chunk_end - chunk_begin) * n_moduli uint32, fully overwritten.
+ *   stream         cudaStream_t (NULL = default stream).  The call does not synchronise; invalid
+ *                  arguments are reported before anything is enqueued; launch errors map to
+ *                  PAIRINGS_ECUDA; asynchronous faults surface at the caller's next synchronise.
+ *   An empty range (chunk_begin == chunk_end) is legal and enqueues nothing.
+ */
+int count_pairings(int kind, int n, int chunk_bits,
+                   uint64_t chunk_begin, uint64_t chunk_end,
+                   const uint32_t* moduli, int n_moduli,
+                   uint32_t* out_residues, void* stream);
+
+/* Launch options for count_pairings_ex.  Zero / NULL in a field means "library default".
+ * The result never depends on these (tests check that); they only change the geometry. */
+typedef struct pairings_launch_opts {
+    int variant;          /* PAIRINGS_VARIANT_* */
+    int gray_bits;        /* g: low index bits each thread walks in Gray-code order */
+    int block_threads;    /* threads per block (multiple of 32) */
+    int blocks_per_chunk; /* power of two; >1 splits one chunk's thread prefixes over several blocks */
+    uint64_t* nonzero_terms; /* DEVICE, optional: one uint64 that receives += number of terms with a
+                                non-zero product (the early-out statistic, §8(a) row a4) */
+} pairings_launch_opts;
+
+enum {
+    PAIRINGS_VARIANT_AUTO = 0,
+    PAIRINGS_VARIANT_GENERIC = 1, /* any (kind, n): int32 pair-sums, boundary-guarded delta rule, one
+                                     Montgomery product chain per modulus and term */
+    PAIRINGS_VARIANT_SWAR = 2     /* specialised (kind, n): byte-packed pair-sums, unrolled Gray blocks,
+                                     warp-level compaction of non-zero terms, exact multi-word
+                                     accumulation reduced modulo the primes once per thread */
+};
+
+int count_pairings_ex(int kind, int n, int chunk_bits,
+                      uint64_t chunk_begin, uint64_t chunk_end,
+                      const uint32_t* moduli, int n_moduli,
+                      uint32_t* out_residues, void* stream,
+                      const pairings_launch_opts* opts /* HOST, may be NULL */);
+
+/* 1 if PAIRINGS_VARIANT_SWAR is compiled for (kind, n), else 0. */
+int pairings_has_swar(int kind, int n);
+
+/* Same computation with a HOST output buffer: allocates the device rows on `stream`
+ * (cudaMallocAsync), launches, copies the rows back and synchronises the stream.  This is the
+ * end-to-end call bench.py times as "e2e".  out_residues_host: (chunk_end-chunk_begin)*n_moduli. */
+int count_pairings_host(int kind, int n, int chunk_bits,
+                        uint64_t chunk_begin, uint64_t chunk_end,
+                        const uint32_t* moduli, int n_moduli,
+                        uint32_t* out_residues_host, void* stream,
+                        const pairings_launch_opts* opts /* HOST, may be NULL */);
+
+/* ------------------------------------------------------------------------------------------------
+ * Host side: moduli, partitioner, journal, row sums, CRT.
+ */
+
+/* The `count` largest primes below 2^31 in descending order (reading A7 of PAPER.md:257 "modulo
+ * number of co-primes"): 2147483647, 2147483629, 2147483587, ...  out: HOST, count <= 16. */
+int pairings_default_moduli(uint32_t* out, int count);
+
+/* Smallest m such that the product of the first m default moduli exceeds 2 * 2^{2n-1} * prod_k (2n-d_k)
+ * >= 2|H| (each |P_k| <= 2n-d_k).  Negative code on invalid (kind, n). */
+int pairings_min_moduli(int kind, int n);
+
+/* Number of CRT moduli the north_star bound (2n)^n * 2^{2n} asks for (>= pairings_min_moduli). */
+int pairings_bound_moduli(int kind, int n);
+
+/* §8(a) row a1 — host prefix partitioner ("split {1,-1}^{2n} sequences into several
+ * independent sets and simply put the result together at the end"; splits are by fixed bits, so
+ * every piece is a power-of-two sub-cube).  Cuts [0, 2^chunk_bits) minus the union of the `n_done`
+ * half-open ranges done[2j], done[2j+1] into ranges of at most max_chunks chunks, in ascending order.
+ * Writes up to cap_ranges pairs to out_ranges (HOST) and returns the number of pairs needed
+ * (which may exceed cap_ranges), or a negative code. */
+int64_t pairings_partition(int chunk_bits, uint64_t max_chunks,
+                           const uint64_t* done, int n_done,
+                           uint64_t* out_ranges, int64_t cap_ranges);
+
+/* The slice of [0, 2^chunk_bits) owned by `rank` of `world` when chunks are dealt out as
+ * contiguous, equal (+-1) ranges — replicas on disjoint ranges are the only multi-GPU mode (§8(e)). */
+int pairings_rank_range(int chunk_bits, int rank, int world, uint64_t* out_begin, uint64_t* out_end);
+
+/* Adds n_rows rows (HOST, row-major n_rows x n_moduli, values < p_i) into total[i] modulo moduli[i].
+ * total (HOST, n_moduli values < p_i) is read and updated. */
+int pairings_sum_rows(const uint32_t* rows, uint64_t n_rows,
+                      const uint32_t* moduli, int n_moduli, uint32_t* total);
+
+/* Resumable journal: an append-only text file.  Header line fixes (kind, n, chunk_bits, moduli);
+ * every further line is "begin end r_0 .. r_{m-1}" = the summed rows of chunks [begin, end).
+ * pairings_journal_append creates the file (with header) if absent and refuses (PAIRINGS_EJOURNAL)
+ * a file written for other parameters.  pairings_journal_load returns the number of recorded
+ * ranges (writing up to cap_ranges (begin,end) pairs) and the sum of their rows in total_out;
+ * a missing file is 0 ranges.  Truncated last lines (a crash mid-write) are ignored. */
+int pairings_journal_append(const char* path, int kind, int n, int chunk_bits,
+                            const uint32_t* moduli, int n_moduli,
+                            uint64_t chunk_begin, uint64_t chunk_end, const uint32_t* row_sum);
+int64_t pairings_journal_load(const char* path, int kind, int n, int chunk_bits,
+                              const uint32_t* moduli, int n_moduli,
+                              uint64_t* out_ranges, int64_t cap_ranges, uint32_t* total_out);
+
+/* Whole-job host driver: partition -> count_pairings_host per range -> sum rows -> journal.
+ * Skips ranges already in the journal (journal_path may be NULL = no journal).  Stops after
+ * max_calls kernel calls if max_calls > 0 (so a run can be interrupted and resumed).
+ * total_out (HOST, n_moduli) = summed residues of every chunk done so far (journal included);
+ * *chunks_done_out = how many of the 2^chunk_bits chunks that covers. */
+int pairings_run(int kind, int n, int chunk_bits,
+                 const uint32_t* moduli, int n_moduli,
+                 uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                 void* stream, const pairings_launch_opts* opts,
+                 uint32_t* total_out, uint64_t* chunks_done_out);
+
+/* §8(a) row a7 — CRT reconstruction ("the actual value is obtained using the chinese
+ * remainder theorem") and the exact division of Lemma 2.1.
+ *   moduli[0..n_moduli-2] are the CRT primes, moduli[n_moduli-1] is the redundant check prime
+ *   (n_moduli >= 2).  total_residues: HOST, H mod p_i summed over all 2^chunk_bits chunks.
+ *   Garner CRT -> H in [0, prod p); H mod check prime must match (else PAIRINGS_ECHECK);
+ *   2^{2n-1} must divide H and D = H / 2^{2n-1} must be even (else PAIRINGS_EINEXACT);
+ *   the CRT product must exceed 2 * 2^{2n-1} * prod_k (2n-d_k) (else PAIRINGS_ERANGE).
+ *   out_distinct_dec    D(n), reflections distinct, decimal, NUL-terminated
+ *   out_identified_dec  D(n)/2, reflections identified (the paper's S(n) / L(n))
+ *   cap                 size of each output buffer (PAIRINGS_ERANGE if too small) */
+int pairings_reconstruct(int kind, int n,
+                         const uint32_t* moduli, int n_moduli,
+                         const uint32_t* total_residues,
+                         char* out_distinct_dec, char* out_identified_dec, size_t cap);
+
+/* Symmetric CRT lift of one row (no check prime, no division): the signed T(c) in (-M/2, M/2]
+ * as a decimal string (reading A8).  For parity tests of single chunks. */
+int pairings_crt_signed(const uint32_t* moduli, int n_moduli, const uint32_t* residues,
+                        char* out_dec, size_t cap);
+
+const char* pairings_strerror(int code);
+
+/* Library build string: version, CUDA arch, compiled SWAR specialisations. */
+const char* pairings_build_info(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAIRINGS_B200_H */

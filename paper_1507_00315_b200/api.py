@@ -1,0 +1,226 @@
+"""ctypes binding for include/pairings.h — same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SO = os.path.join(_HERE, "libpairings_b200.so")
+
+SKOLEM, LANGFORD = 0, 1
+VARIANT_AUTO, VARIANT_GENERIC, VARIANT_SWAR = 0, 1, 2
+_CAP = 256
+
+u32p = ctypes.POINTER(ctypes.c_uint32)
+u64p = ctypes.POINTER(ctypes.c_uint64)
+
+
+class LaunchOpts(ctypes.Structure):
+    """struct pairings_launch_opts (include/pairings.h)."""
+    _fields_ = [("variant", ctypes.c_int), ("gray_bits", ctypes.c_int), ("block_threads", ctypes.c_int),
+                ("blocks_per_chunk", ctypes.c_int), ("nonzero_terms", ctypes.c_void_p)]
+
+
+class PairingsError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        super().__init__("%s: %s (code %d)" % (where, pairings_strerror(code), code))
+
+
+_lib = None
+
+
+def library_path() -> str:
+    return _SO
+
+
+def lib():
+    """Loads libpairings_b200.so; fails loudly if it has not been built (python -m paper_1507_00315_b200.build)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_SO):
+        raise ImportError("libpairings_b200.so is missing at %s — build it with "
+                          "`python -m paper_1507_00315_b200.build` (there is no CPU fallback)" % _SO)
+    L = ctypes.CDLL(_SO)
+    i, u64, vp, cp = ctypes.c_int, ctypes.c_uint64, ctypes.c_void_p, ctypes.c_char_p
+    optp = ctypes.POINTER(LaunchOpts)
+    sigs = {
+        "count_pairings": (i, [i, i, i, u64, u64, u32p, i, vp, vp]),
+        "count_pairings_ex": (i, [i, i, i, u64, u64, u32p, i, vp, vp, optp]),
+        "count_pairings_host": (i, [i, i, i, u64, u64, u32p, i, u32p, vp, optp]),
+        "pairings_has_swar": (i, [i, i]),
+        "pairings_default_moduli": (i, [u32p, i]),
+        "pairings_min_moduli": (i, [i, i]),
+        "pairings_bound_moduli": (i, [i, i]),
+        "pairings_partition": (ctypes.c_int64, [i, u64, u64p, i, u64p, ctypes.c_int64]),
+        "pairings_rank_range": (i, [i, i, i, u64p, u64p]),
+        "pairings_sum_rows": (i, [u32p, u64, u32p, i, u32p]),
+        "pairings_journal_append": (i, [cp, i, i, i, u32p, i, u64, u64, u32p]),
+        "pairings_journal_load": (ctypes.c_int64, [cp, i, i, i, u32p, i, u64p, ctypes.c_int64, u32p]),
+        "pairings_run": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, u32p, u64p]),
+        "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
+        "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
+        "pairings_strerror": (cp, [i]),
+        "pairings_build_info": (cp, []),
+    }
+    for name, (res, args) in sigs.items():
+        fn = getattr(L, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _u32(values: Sequence[int]):
+    return (ctypes.c_uint32 * max(len(values), 1))(*values)
+
+
+def _opts(opts: Optional[LaunchOpts]):
+    return ctypes.byref(opts) if opts is not None else None
+
+
+def _check(rc: int, where: str):
+    if rc < 0:
+        raise PairingsError(int(rc), where)
+    return rc
+
+
+def pairings_strerror(code: int) -> str:
+    return lib().pairings_strerror(int(code)).decode()
+
+
+def pairings_build_info() -> str:
+    return lib().pairings_build_info().decode()
+
+
+def pairings_has_swar(kind: int, n: int) -> bool:
+    return bool(lib().pairings_has_swar(kind, n))
+
+
+def count_pairings(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, out_residues_ptr: int, stream: int = 0):
+    """out_residues_ptr: DEVICE pointer (int, e.g. tensor.data_ptr()); stream: cudaStream_t as int."""
+    m = _u32(moduli)
+    _check(lib().count_pairings(kind, n, chunk_bits, chunk_begin, chunk_end, m, len(moduli),
+                                ctypes.c_void_p(out_residues_ptr), ctypes.c_void_p(stream)), "count_pairings")
+
+
+def count_pairings_ex(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, out_residues_ptr: int, stream: int = 0,
+                      opts: Optional[LaunchOpts] = None):
+    m = _u32(moduli)
+    _check(lib().count_pairings_ex(kind, n, chunk_bits, chunk_begin, chunk_end, m, len(moduli),
+                                   ctypes.c_void_p(out_residues_ptr), ctypes.c_void_p(stream), _opts(opts)),
+           "count_pairings_ex")
+
+
+def count_pairings_host(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, stream: int = 0,
+                        opts: Optional[LaunchOpts] = None, out=None):
+    """Returns the rows as a list of lists (or fills `out`, a ctypes uint32 array, and returns it)."""
+    m = _u32(moduli)
+    rows = chunk_end - chunk_begin
+    ret_list = out is None
+    if out is None:
+        out = (ctypes.c_uint32 * max(rows * len(moduli), 1))()
+    _check(lib().count_pairings_host(kind, n, chunk_bits, chunk_begin, chunk_end, m, len(moduli), out,
+                                     ctypes.c_void_p(stream), _opts(opts)), "count_pairings_host")
+    if not ret_list:
+        return out
+    k = len(moduli)
+    return [[int(out[r * k + j]) for j in range(k)] for r in range(rows)]
+
+
+def pairings_default_moduli(count: int):
+    out = (ctypes.c_uint32 * max(count, 1))()
+    _check(lib().pairings_default_moduli(out, count), "pairings_default_moduli")
+    return [int(out[j]) for j in range(count)]
+
+
+def pairings_min_moduli(kind: int, n: int) -> int:
+    return _check(lib().pairings_min_moduli(kind, n), "pairings_min_moduli")
+
+
+def pairings_bound_moduli(kind: int, n: int) -> int:
+    return _check(lib().pairings_bound_moduli(kind, n), "pairings_bound_moduli")
+
+
+def pairings_partition(chunk_bits: int, max_chunks: int, done=()):
+    flat = [v for r in done for v in r]
+    d = (ctypes.c_uint64 * max(len(flat), 1))(*flat)
+    need = _check(lib().pairings_partition(chunk_bits, max_chunks, d, len(done), None, 0), "pairings_partition")
+    out = (ctypes.c_uint64 * max(2 * need, 1))()
+    _check(lib().pairings_partition(chunk_bits, max_chunks, d, len(done), out, need), "pairings_partition")
+    return [(int(out[2 * j]), int(out[2 * j + 1])) for j in range(need)]
+
+
+def pairings_rank_range(chunk_bits: int, rank: int, world: int):
+    b, e = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    _check(lib().pairings_rank_range(chunk_bits, rank, world, ctypes.byref(b), ctypes.byref(e)), "pairings_rank_range")
+    return int(b.value), int(e.value)
+
+
+def pairings_sum_rows(rows, moduli, total=None):
+    """rows: list of rows or a flat ctypes uint32 array (then pass n_rows via len(rows)//len(moduli))."""
+    k = len(moduli)
+    if isinstance(rows, ctypes.Array):
+        flat, n_rows = rows, len(rows) // k
+    else:
+        vals = [v for r in rows for v in r]
+        flat, n_rows = _u32(vals), len(rows)
+    t = _u32(list(total) if total is not None else [0] * k)
+    _check(lib().pairings_sum_rows(flat, n_rows, _u32(moduli), k, t), "pairings_sum_rows")
+    return [int(t[j]) for j in range(k)]
+
+
+def pairings_journal_append(path, kind, n, chunk_bits, moduli, chunk_begin, chunk_end, row_sum):
+    _check(lib().pairings_journal_append(os.fsencode(path), kind, n, chunk_bits, _u32(moduli), len(moduli),
+                                         chunk_begin, chunk_end, _u32(row_sum)), "pairings_journal_append")
+
+
+def pairings_journal_load(path, kind, n, chunk_bits, moduli):
+    k = len(moduli)
+    t = _u32([0] * k)
+    need = _check(lib().pairings_journal_load(os.fsencode(path), kind, n, chunk_bits, _u32(moduli), k, None, 0, t),
+                  "pairings_journal_load")
+    out = (ctypes.c_uint64 * max(2 * need, 1))()
+    _check(lib().pairings_journal_load(os.fsencode(path), kind, n, chunk_bits, _u32(moduli), k, out, need, t),
+           "pairings_journal_load")
+    return [(int(out[2 * j]), int(out[2 * j + 1])) for j in range(need)], [int(t[j]) for j in range(k)]
+
+
+def pairings_run(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=None, max_calls=0, stream: int = 0,
+                 opts: Optional[LaunchOpts] = None):
+    """Whole-job host driver.  Returns (total residues, chunks done)."""
+    k = len(moduli)
+    t = _u32([0] * k)
+    done = ctypes.c_uint64(0)
+    jp = os.fsencode(journal_path) if journal_path is not None else None
+    _check(lib().pairings_run(kind, n, chunk_bits, _u32(moduli), k, chunks_per_call, jp, max_calls,
+                              ctypes.c_void_p(stream), _opts(opts), t, ctypes.byref(done)), "pairings_run")
+    return [int(t[j]) for j in range(k)], int(done.value)
+
+
+def pairings_reconstruct(kind, n, moduli, total_residues):
+    """Returns (D, S) = (reflections distinct, reflections identified) as Python ints."""
+    a, b = ctypes.create_string_buffer(_CAP), ctypes.create_string_buffer(_CAP)
+    _check(lib().pairings_reconstruct(kind, n, _u32(moduli), len(moduli), _u32(total_residues), a, b, _CAP),
+           "pairings_reconstruct")
+    return int(a.value), int(b.value)
+
+
+def pairings_crt_signed(moduli, residues) -> int:
+    a = ctypes.create_string_buffer(_CAP)
+    _check(lib().pairings_crt_signed(_u32(moduli), len(moduli), _u32(residues), a, _CAP), "pairings_crt_signed")
+    return int(a.value)
+
+
+def count(kind: int, n: int, chunk_bits: Optional[int] = None, n_moduli: Optional[int] = None,
+          chunks_per_call: int = 1 << 12, journal_path=None, opts: Optional[LaunchOpts] = None):
+    """Convenience: the whole path for (kind, n) -> (D, S).  Calls only the C ABI."""
+    if n_moduli is None:
+        n_moduli = pairings_bound_moduli(kind, n) + 1
+    moduli = pairings_default_moduli(n_moduli)
+    if chunk_bits is None:
+        chunk_bits = max(0, min(2 * n - 1 - 17, 20))
+    total, done = pairings_run(kind, n, chunk_bits, moduli, chunks_per_call, journal_path, 0, 0, opts)
+    assert done == 1 << chunk_bits
+    return pairings_reconstruct(kind, n, moduli, total)

@@ -1,0 +1,393 @@
+// count_pairings: argument validation, Montgomery constants, launch geometry, the GENERIC kernel
+// (any kind, any 2 <= n <= 32), the host-buffer variant and the whole-job host driver.
+//
+// The generic kernel is north_star's description taken literally:
+//   a2  each thread evaluates its prefix's n pair-sums directly (popcount of X ^ (X >> d_k)),
+//   a3  walks its low g bits in binary-reflected Gray-code order, updating every
+//       P_k by  -2 x_j (x_{j-d_k} + x_{j+d_k})  with both neighbours boundary-guarded,
+//   a4  skips terms with a zero factor,
+//   a5  multiplies the rest as exact <= 60-bit group products and one 32-bit Montgomery chain per
+//       modulus ("calculations modulo number of co-primes"),
+//   a6  reduces per thread -> warp shuffles -> shared memory -> one row per chunk.
+// The specialised SWAR kernels (swar_kernel.cuh) are the fast path; this one is the fallback for
+// every (kind, n) they are not compiled for and an independent second implementation of the rows.
+#include "pairings.h"
+#include "internal.h"
+
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+namespace pairings {
+
+// ------------------------------------------------------------------------------------------------
+// host: Montgomery constants
+// ------------------------------------------------------------------------------------------------
+static MontPrime make_prime(uint32_t p) {
+    MontPrime mp; std::memset(&mp, 0, sizeof mp);
+    mp.p = p;
+    uint32_t inv = p;                                  // Newton: inv = p^{-1} mod 2^32 (p odd; 3 correct bits to start)
+    for (int i = 0; i < 5; i++) inv *= 2u - p * inv;
+    mp.pinv_neg = 0u - inv;
+    uint64_t r = 1;
+    for (int i = 0; i < 32; i++) r = (r * 2) % p;
+    mp.r1 = (uint32_t)r;
+    for (int i = 0; i < 32; i++) r = (r * 2) % p;
+    mp.r2 = (uint32_t)r;
+    for (int i = 0; i < 32; i++) r = (r * 2) % p;
+    mp.r3 = (uint32_t)r;
+    return mp;
+}
+
+// ------------------------------------------------------------------------------------------------
+// device helpers
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t montmul(uint32_t a, uint32_t b, uint32_t p, uint32_t pinv_neg) {
+    // a*b < p*2^32  ->  returns a*b*2^{-32} mod p in [0,p)
+    const uint64_t t = (uint64_t)a * b;
+    const uint32_t m = (uint32_t)t * pinv_neg;
+    const uint32_t u = (uint32_t)((t + (uint64_t)m * p) >> 32);   // < 2p < 2^32
+    return u >= p ? u - p : u;
+}
+
+// Montgomery form (value * 2^32 mod p) of a signed 64-bit integer with |g| < 2^62
+__device__ __forceinline__ uint32_t to_mont64(long long g, const MontPrime& mp) {
+    const bool neg = g < 0;
+    const unsigned long long a = neg ? 0ULL - (unsigned long long)g : (unsigned long long)g;
+    uint32_t r = montmul((uint32_t)a, mp.r2, mp.p, mp.pinv_neg) + montmul((uint32_t)(a >> 32), mp.r3, mp.p, mp.pinv_neg);
+    if (r >= mp.p) r -= mp.p;
+    if (neg && r) r = mp.p - r;
+    return r;
+}
+
+// out[idx] = (out[idx] + v) mod p, atomically (several blocks may share one chunk row)
+__device__ __forceinline__ void atomic_add_mod(uint32_t* addr, uint32_t v, uint32_t p) {
+    uint32_t old = *addr, assumed;
+    do {
+        assumed = old;
+        uint32_t s = assumed + v; if (s >= p) s -= p;
+        old = atomicCAS(addr, assumed, s);
+    } while (old != assumed);
+}
+
+// Block-level sum of per-thread residues (Montgomery or plain, already < p) and the row write.
+// vals[i] < p_i.  red: shared scratch of (blockDim/32) * PAIRINGS_MAX_MODULI uint64.
+__device__ __forceinline__ void block_reduce_write(const KernelParams& kp, const uint32_t* vals,
+                                                   unsigned long long nz, unsigned long long* red,
+                                                   uint64_t chunk_local) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    for (int i = 0; i < kp.n_moduli; i++) {
+        unsigned long long v = vals[i];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+        if (lane == 0) red[warp * PAIRINGS_MAX_MODULI + i] = v;
+    }
+    for (int o = 16; o > 0; o >>= 1) nz += __shfl_xor_sync(0xffffffffu, nz, o);
+    if (lane == 0 && kp.nonzero && nz) atomicAdd(kp.nonzero, nz);
+    __syncthreads();
+    if ((int)threadIdx.x < kp.n_moduli) {
+        const int i = threadIdx.x;
+        unsigned long long s = 0;
+        for (int w = 0; w < nwarps; w++) s += red[w * PAIRINGS_MAX_MODULI + i];
+        const uint32_t p = kp.primes[i].p;
+        const uint32_t r = (uint32_t)(s % p);
+        uint32_t* dst = kp.out + chunk_local * (uint64_t)kp.n_moduli + (uint64_t)i;
+        if (kp.log2_bpc == 0) *dst = r; else atomic_add_mod(dst, r, p);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// GENERIC kernel
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+generic_kernel(const __grid_constant__ KernelParams kp) {
+    __shared__ unsigned long long red[8 * PAIRINGS_MAX_MODULI];
+    const int n = kp.n, N = 2 * n, B = N - 1, C = kp.chunk_bits, g = kp.gray_bits;
+    const int kind = kp.kind, M = kp.n_moduli;
+    const uint64_t chunk_local = (uint64_t)blockIdx.x >> kp.log2_bpc;
+    const uint64_t sub = (uint64_t)blockIdx.x & ((1ULL << kp.log2_bpc) - 1);
+    const uint64_t chunk = kp.chunk_begin + chunk_local;
+    const int tb = B - C;                               // index bits inside one chunk
+    const uint64_t prefixes = 1ULL << (tb - g);          // thread prefixes per chunk
+    const uint64_t per_block = prefixes >> kp.log2_bpc;  // >= 1 by construction
+    const uint64_t chunk_base = (tb >= 64) ? 0 : (chunk << tb);
+
+    unsigned long long acc[PAIRINGS_MAX_MODULI];
+#pragma unroll
+    for (int i = 0; i < PAIRINGS_MAX_MODULI; i++) acc[i] = 0;
+    unsigned long long nz = 0;
+
+    for (uint64_t q = sub * per_block + threadIdx.x; q < (sub + 1) * per_block; q += blockDim.x) {
+        uint64_t V = chunk_base | (q << g);             // bit b <-> position N-b, set <-> x = -1
+        int P[32];
+#pragma unroll
+        for (int k = 1; k <= 32; k++) {
+            P[k - 1] = 1;
+            if (k <= n) {
+                const int d = dist(kind, k), cnt = N - d;          // cnt summands, 1 <= cnt <= 63
+                const uint64_t mask = (1ULL << cnt) - 1;
+                P[k - 1] = cnt - 2 * __popcll((V ^ (V >> d)) & mask);
+            }
+        }
+        int sign = (__popcll(V) & 1) ? -1 : 1;
+        const uint64_t steps = 1ULL << g;
+        for (uint64_t t = 0; t < steps; t++) {
+            // ---- a4: zero-factor test, a5: signed product -> residues
+            bool zero = false;
+#pragma unroll
+            for (int k = 0; k < 32; k++) zero |= (P[k] == 0);
+            if (!zero) {
+                nz++;
+                long long G0 = sign, G1 = 1, G2 = 1, G3 = 1;       // <= 10 factors of |P| <= 63 each: < 2^60
+#pragma unroll
+                for (int k = 0; k < 32; k++) {
+                    if (k < 10) G0 *= P[k]; else if (k < 20) G1 *= P[k]; else if (k < 30) G2 *= P[k]; else G3 *= P[k];
+                }
+                for (int i = 0; i < M; i++) {
+                    const MontPrime& mp = kp.primes[i];
+                    uint32_t r = to_mont64(G0, mp);
+                    if (n > 10) r = montmul(r, to_mont64(G1, mp), mp.p, mp.pinv_neg);
+                    if (n > 20) r = montmul(r, to_mont64(G2, mp), mp.p, mp.pinv_neg);
+                    if (n > 30) r = montmul(r, to_mont64(G3, mp), mp.p, mp.pinv_neg);
+                    acc[i] += r;                                  // Montgomery form, < p < 2^31
+                }
+            }
+            // ---- a3: Gray step t -> t+1 flips index bit ctz(t+1), i.e. position j = N - b
+            if (t + 1 < steps) {
+                const int b = __ffsll((long long)(t + 1)) - 1;
+                const int xj = 1 - 2 * (int)((V >> b) & 1ULL);
+#pragma unroll
+                for (int k = 1; k <= 32; k++) {
+                    if (k <= n) {
+                        const int d = dist(kind, k);
+                        int nb = 0;
+                        if (b + d <= N - 1) nb += 1 - 2 * (int)((V >> (b + d)) & 1ULL);   // x_{j-d}, exists iff j-d >= 1
+                        if (b - d >= 0) nb += 1 - 2 * (int)((V >> (b - d)) & 1ULL);       // x_{j+d}, exists iff j+d <= N
+                        P[k - 1] -= 2 * xj * nb;
+                    }
+                }
+                V ^= 1ULL << b;
+                sign = -sign;
+            }
+        }
+        // keep the 64-bit accumulators far from overflow across prefixes
+#pragma unroll
+        for (int i = 0; i < PAIRINGS_MAX_MODULI; i++) if (i < M && acc[i] >= (1ULL << 62)) acc[i] %= kp.primes[i].p;
+    }
+
+    uint32_t vals[PAIRINGS_MAX_MODULI];
+#pragma unroll
+    for (int i = 0; i < PAIRINGS_MAX_MODULI; i++) {
+        vals[i] = 0;
+        if (i < M) {
+            const MontPrime& mp = kp.primes[i];
+            vals[i] = montmul((uint32_t)(acc[i] % mp.p), 1u, mp.p, mp.pinv_neg);   // out of Montgomery form
+        }
+    }
+    block_reduce_write(kp, vals, nz, red, chunk_local);
+}
+
+// ------------------------------------------------------------------------------------------------
+// host: geometry + launch
+// ------------------------------------------------------------------------------------------------
+static int ilog2_floor(uint64_t v) { int r = 0; while (v >>= 1) r++; return r; }
+static bool is_pow2(uint64_t v) { return v && !(v & (v - 1)); }
+
+struct Geometry { int variant, g, threads, log2_bpc; };
+
+static int choose_geometry(int kind, int n, int chunk_bits, uint64_t n_chunks,
+                           const pairings_launch_opts* o, Geometry* out) {
+    const int tb = 2 * n - 1 - chunk_bits;
+    int variant = o ? o->variant : PAIRINGS_VARIANT_AUTO;
+    if (variant < 0 || variant > PAIRINGS_VARIANT_SWAR) return PAIRINGS_EINVAL_OPTS;
+    const int h = swar_min_gray_bits();
+    const bool swar_ok = swar_lookup(kind, n) != nullptr && tb >= h && n - 2 >= h;
+    if (variant == PAIRINGS_VARIANT_SWAR && !swar_ok) return PAIRINGS_EINVAL_OPTS;
+    if (variant == PAIRINGS_VARIANT_AUTO) variant = swar_ok ? PAIRINGS_VARIANT_SWAR : PAIRINGS_VARIANT_GENERIC;
+
+    const int gmin = variant == PAIRINGS_VARIANT_SWAR ? h : 0;
+    const int gmax = variant == PAIRINGS_VARIANT_SWAR ? std::min(tb, n - 2) : std::min(tb, 40);
+    int g = o ? o->gray_bits : 0;
+    if (g != 0) { if (g < gmin || g > gmax) return PAIRINGS_EINVAL_OPTS; }
+    else {
+        // default: enough thread prefixes to fill 148 SMs x 2048 threads a few times over, but at
+        // least 2^10 terms per prefix when the problem is big enough to afford it.
+        const int total_bits = tb + ilog2_floor(std::max<uint64_t>(n_chunks, 1));
+        g = total_bits - 20;
+        g = std::max(g, gmin); g = std::min(g, std::min(gmax, variant == PAIRINGS_VARIANT_SWAR ? 14 : 12));
+        g = std::max(g, gmin);
+    }
+    int threads = o ? o->block_threads : 0;
+    if (threads != 0) { if (threads < 32 || threads > 256 || threads % 32) return PAIRINGS_EINVAL_OPTS; }
+    else {
+        threads = 256;
+        const int pb = tb - g;                           // log2(prefixes per chunk)
+        if (pb < 8) threads = std::max(32, 1 << pb);
+    }
+    int bpc = o ? o->blocks_per_chunk : 0;
+    const uint64_t prefixes = 1ULL << std::min(tb - g, 62);
+    if (bpc != 0) { if (!is_pow2((uint64_t)bpc) || (uint64_t)bpc > prefixes || bpc > (1 << 20)) return PAIRINGS_EINVAL_OPTS; }
+    else {
+        bpc = 1;
+        const uint64_t want_blocks = 148ULL * 16;        // a few waves
+        while (n_chunks * (uint64_t)bpc < want_blocks && (uint64_t)bpc * 2 * (uint64_t)threads <= prefixes && bpc < (1 << 20)) bpc *= 2;
+    }
+    out->variant = variant; out->g = g; out->threads = threads; out->log2_bpc = ilog2_floor((uint64_t)bpc);
+    return PAIRINGS_OK;
+}
+
+static int validate(int kind, int n, int chunk_bits, uint64_t b, uint64_t e, const uint32_t* moduli, int n_moduli, const void* out) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    rc = check_chunks(n, chunk_bits, b, e); if (rc) return rc;
+    rc = check_moduli(moduli, n_moduli); if (rc) return rc;
+    if (!out && e > b) return PAIRINGS_ENULL;
+    return PAIRINGS_OK;
+}
+
+static int launch_range(int kind, int n, int chunk_bits, uint64_t chunk_begin, uint64_t chunk_end,
+                        const uint32_t* moduli, int n_moduli, uint32_t* out, cudaStream_t stream,
+                        const pairings_launch_opts* opts) {
+    const uint64_t n_chunks = chunk_end - chunk_begin;
+    if (n_chunks == 0) return PAIRINGS_OK;
+    Geometry geo;
+    int rc = choose_geometry(kind, n, chunk_bits, n_chunks, opts, &geo); if (rc) return rc;
+
+    KernelParams kp; std::memset(&kp, 0, sizeof kp);
+    kp.kind = kind; kp.n = n; kp.chunk_bits = chunk_bits; kp.gray_bits = geo.g; kp.log2_bpc = geo.log2_bpc;
+    kp.n_moduli = n_moduli;
+    kp.nonzero = opts ? (unsigned long long*)opts->nonzero_terms : nullptr;
+    for (int i = 0; i < n_moduli; i++) kp.primes[i] = make_prime(moduli[i]);
+
+    (void)cudaGetLastError();
+    if (geo.log2_bpc > 0) {
+        if (cudaMemsetAsync(out, 0, n_chunks * (uint64_t)n_moduli * sizeof(uint32_t), stream) != cudaSuccess) {
+            (void)cudaGetLastError(); return PAIRINGS_ECUDA;
+        }
+    }
+    // at most 2^30 blocks per launch
+    const uint64_t max_chunks_per_launch = std::max<uint64_t>(1, (1ULL << 30) >> geo.log2_bpc);
+    swar_launch_fn swar = geo.variant == PAIRINGS_VARIANT_SWAR ? swar_lookup(kind, n) : nullptr;
+    for (uint64_t off = 0; off < n_chunks; off += max_chunks_per_launch) {
+        const uint64_t cnt = std::min(max_chunks_per_launch, n_chunks - off);
+        kp.chunk_begin = chunk_begin + off; kp.n_chunks = cnt;
+        kp.out = out + off * (uint64_t)n_moduli;
+        const unsigned grid = (unsigned)(cnt << geo.log2_bpc);
+        cudaError_t err;
+        if (swar) err = (cudaError_t)swar(kp, geo.threads, grid, (void*)stream);
+        else { generic_kernel<<<grid, geo.threads, 0, stream>>>(kp); err = cudaGetLastError(); }
+        if (err != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    }
+    return PAIRINGS_OK;
+}
+
+}  // namespace pairings
+
+using namespace pairings;
+
+extern "C" {
+
+int count_pairings_ex(int kind, int n, int chunk_bits, uint64_t chunk_begin, uint64_t chunk_end,
+                      const uint32_t* moduli, int n_moduli, uint32_t* out_residues, void* stream,
+                      const pairings_launch_opts* opts) {
+    int rc = validate(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, out_residues); if (rc) return rc;
+    return launch_range(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, out_residues, (cudaStream_t)stream, opts);
+}
+
+int count_pairings(int kind, int n, int chunk_bits, uint64_t chunk_begin, uint64_t chunk_end,
+                   const uint32_t* moduli, int n_moduli, uint32_t* out_residues, void* stream) {
+    return count_pairings_ex(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, out_residues, stream, nullptr);
+}
+
+int pairings_has_swar(int kind, int n) {
+    if (check_kind_n(kind, n)) return 0;
+    return swar_lookup(kind, n) != nullptr ? 1 : 0;
+}
+
+int count_pairings_host(int kind, int n, int chunk_bits, uint64_t chunk_begin, uint64_t chunk_end,
+                        const uint32_t* moduli, int n_moduli, uint32_t* out_residues_host, void* stream,
+                        const pairings_launch_opts* opts) {
+    int rc = validate(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, out_residues_host); if (rc) return rc;
+    const uint64_t n_chunks = chunk_end - chunk_begin;
+    if (n_chunks == 0) return PAIRINGS_OK;
+    {   // options are validated before anything is allocated
+        Geometry geo; rc = choose_geometry(kind, n, chunk_bits, n_chunks, opts, &geo); if (rc) return rc;
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = n_chunks * (size_t)n_moduli * sizeof(uint32_t);
+    uint32_t* dev = nullptr;
+    (void)cudaGetLastError();
+    if (cudaMallocAsync((void**)&dev, bytes, s) != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    rc = launch_range(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, dev, s, opts);
+    cudaError_t e1 = cudaSuccess;
+    if (rc == PAIRINGS_OK) e1 = cudaMemcpyAsync(out_residues_host, dev, bytes, cudaMemcpyDeviceToHost, s);
+    cudaError_t e2 = cudaFreeAsync(dev, s);
+    cudaError_t e3 = cudaStreamSynchronize(s);
+    if (rc) return rc;
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    return PAIRINGS_OK;
+}
+
+int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                 uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                 void* stream, const pairings_launch_opts* opts,
+                 uint32_t* total_out, uint64_t* chunks_done_out) {
+    int rc = validate(kind, n, chunk_bits, 0, 0, moduli, n_moduli, total_out); if (rc) return rc;
+    if (!total_out || !chunks_done_out) return PAIRINGS_ENULL;
+    if (chunks_per_call == 0) return PAIRINGS_EINVAL_CHUNK;
+    for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
+    *chunks_done_out = 0;
+
+    // a1: what is already journalled
+    std::vector<uint64_t> done;
+    if (journal_path) {
+        uint32_t jt[PAIRINGS_MAX_MODULI];
+        int64_t nd = pairings_journal_load(journal_path, kind, n, chunk_bits, moduli, n_moduli, nullptr, 0, jt);
+        if (nd < 0) return (int)nd;
+        done.resize((size_t)(2 * nd) + 2);
+        nd = pairings_journal_load(journal_path, kind, n, chunk_bits, moduli, n_moduli, done.data(), nd, total_out);
+        if (nd < 0) return (int)nd;
+        done.resize((size_t)(2 * nd));
+        for (int64_t j = 0; j < nd; j++) *chunks_done_out += done[(size_t)(2 * j + 1)] - done[(size_t)(2 * j)];
+    }
+    // a1: the remaining ranges
+    int64_t need = pairings_partition(chunk_bits, chunks_per_call, done.data(), (int)(done.size() / 2), nullptr, 0);
+    if (need < 0) return (int)need;
+    std::vector<uint64_t> ranges((size_t)(2 * need) + 2);
+    need = pairings_partition(chunk_bits, chunks_per_call, done.data(), (int)(done.size() / 2), ranges.data(), need);
+    if (need < 0) return (int)need;
+
+    std::vector<uint32_t> rows;
+    int64_t calls = 0;
+    for (int64_t r = 0; r < need; r++) {
+        if (max_calls > 0 && calls >= max_calls) break;
+        const uint64_t b = ranges[(size_t)(2 * r)], e = ranges[(size_t)(2 * r + 1)];
+        rows.resize((size_t)(e - b) * (size_t)n_moduli);
+        rc = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, rows.data(), stream, opts);
+        if (rc) return rc;
+        uint32_t row_sum[PAIRINGS_MAX_MODULI] = {0};
+        rc = pairings_sum_rows(rows.data(), e - b, moduli, n_moduli, row_sum); if (rc) return rc;
+        if (journal_path) {
+            rc = pairings_journal_append(journal_path, kind, n, chunk_bits, moduli, n_moduli, b, e, row_sum);
+            if (rc) return rc;
+        }
+        rc = pairings_sum_rows(row_sum, 1, moduli, n_moduli, total_out); if (rc) return rc;
+        *chunks_done_out += e - b;
+        calls++;
+    }
+    return PAIRINGS_OK;
+}
+
+const char* pairings_build_info(void) {
+    static const std::string info = [] {
+        char buf[512];
+        std::snprintf(buf, sizeof buf, "pairings_b200 0.1 sm_100a cuda %d swar[h=%d]: %s", CUDART_VERSION,
+                      swar_min_gray_bits(), swar_list());
+        return std::string(buf);
+    }();
+    return info.c_str();
+}
+
+}  // extern "C"

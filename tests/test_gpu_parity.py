@@ -1,0 +1,194 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on the
+same chunks; totals against backtracking / the paper's printed values.  Integer work: bit-exact,
+zero tolerance."""
+import ctypes
+import threading
+
+import pytest
+
+import oracle
+import paper_1507_00315_b200 as pb
+from paper_1507_00315_b200 import seeds
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+S, L = pb.SKOLEM, pb.LANGFORD
+VARIANTS = [pb.VARIANT_GENERIC, pb.VARIANT_SWAR]
+
+
+def gpu_rows(kind, n, C, begin, end, moduli, opts=None, count_nonzero=False):
+    m = len(moduli)
+    out = torch.full((max(end - begin, 1), m), -1, dtype=torch.int32, device="cuda")
+    nz = torch.zeros(1, dtype=torch.int64, device="cuda")
+    if opts is None:
+        opts = pb.LaunchOpts()
+    if count_nonzero:
+        opts.nonzero_terms = nz.data_ptr()
+    stream = torch.cuda.current_stream().cuda_stream
+    pb.count_pairings_ex(kind, n, C, begin, end, moduli, out.data_ptr(), stream, opts)
+    torch.cuda.synchronize()
+    rows = (out.cpu().to(torch.int64) & 0xFFFFFFFF).tolist()[: end - begin]
+    return (rows, int(nz.item())) if count_nonzero else rows
+
+
+def oracle_rows(kind, n, C, chunks, moduli, threads=8):
+    out = [None] * len(chunks)
+
+    def work(tid):
+        for i in range(tid, len(chunks), threads):
+            out[i] = oracle.chunk(kind, n, C, chunks[i], moduli)
+
+    ts = [threading.Thread(target=work, args=(t,)) for t in range(threads)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    return out
+
+
+def variant_available(variant, kind, n, C):
+    if variant == pb.VARIANT_SWAR:
+        return pb.pairings_has_swar(kind, n) and (2 * n - 1 - C) >= 4
+    return True
+
+
+# ------------------------------------------------------------------------------------------------
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("kind,n,C", [(L, 12, 0), (L, 12, 6), (L, 12, 10), (S, 13, 8), (S, 12, 7), (L, 11, 5)])
+def test_every_chunk_matches_oracle(kind, n, C, variant):
+    if not variant_available(variant, kind, n, C):
+        pytest.skip("variant not compiled for this (kind, n)")
+    moduli = pb.pairings_default_moduli(4)
+    rows, nz = gpu_rows(kind, n, C, 0, 1 << C, moduli, pb.LaunchOpts(variant=variant), count_nonzero=True)
+    want = oracle_rows(kind, n, C, list(range(1 << C)), moduli)
+    for c in range(1 << C):
+        assert rows[c] == want[c][2], (c, rows[c], want[c][2])
+        # symmetric CRT lift of the row equals the oracle's exact signed T(c) (reading A8)
+        assert pb.pairings_crt_signed(moduli, rows[c]) == want[c][0]
+    assert nz == sum(w[1] for w in want)           # early-out statistic phi
+    total = pb.pairings_sum_rows(rows, moduli)
+    D, Sid = pb.pairings_reconstruct(kind, n, moduli, total)
+    assert D == oracle.brute_count(kind, n) and Sid * 2 == D
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("kind,n", [(k, n) for k in (S, L) for n in range(2, 12)])
+def test_small_n_totals_match_backtracking(kind, n, variant, paper_counts):
+    C = max(0, min(5, 2 * n - 1 - 4))
+    if not variant_available(variant, kind, n, C):
+        pytest.skip("variant not compiled for this (kind, n)")
+    moduli = pb.pairings_default_moduli(3)
+    rows = gpu_rows(kind, n, C, 0, 1 << C, moduli, pb.LaunchOpts(variant=variant))
+    D, Sid = pb.pairings_reconstruct(kind, n, moduli, pb.pairings_sum_rows(rows, moduli))
+    assert D == oracle.brute_count(kind, n)
+    if (kind, n) in paper_counts:
+        assert Sid == paper_counts[(kind, n)]
+    else:
+        assert D == 0                                # no pairing exists
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_geometry_never_changes_the_rows(variant):
+    kind, n, C = L, 12, 6
+    if not variant_available(variant, kind, n, C):
+        pytest.skip("variant not compiled")
+    moduli = pb.pairings_default_moduli(4)
+    ref = gpu_rows(kind, n, C, 0, 1 << C, moduli, pb.LaunchOpts(variant=variant))
+    gs = [4, 7, 10] if variant == pb.VARIANT_SWAR else [0, 1, 5, 12, 17]
+    for g in gs:
+        for threads, bpc in ((32, 1), (128, 2), (256, 1), (64, 8)):
+            if bpc * threads > (1 << (2 * n - 1 - C - g)) and bpc > 1:
+                continue
+            o = pb.LaunchOpts(variant=variant, gray_bits=g, block_threads=threads, blocks_per_chunk=bpc)
+            assert gpu_rows(kind, n, C, 0, 1 << C, moduli, o) == ref, (g, threads, bpc)
+    # cutting [0, 2^C) into several calls gives the same rows
+    parts = gpu_rows(kind, n, C, 0, 5, moduli) + gpu_rows(kind, n, C, 5, 5, moduli) + \
+        gpu_rows(kind, n, C, 5, 64, moduli)
+    assert parts == ref
+    # another prime set reconstructs the same integers
+    other = pb.pairings_default_moduli(9)[5:9]
+    rows2 = gpu_rows(kind, n, C, 0, 1 << C, other, pb.LaunchOpts(variant=variant))
+    for c in range(1 << C):
+        assert pb.pairings_crt_signed(other, rows2[c]) == pb.pairings_crt_signed(moduli, ref[c])
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_total_independent_of_chunk_bits(variant):
+    kind, n = S, 12
+    moduli = pb.pairings_default_moduli(4)
+    totals = set()
+    for C in (0, 3, 9, 14, 19):
+        if not variant_available(variant, kind, n, C):
+            continue
+        rows = gpu_rows(kind, n, C, 0, 1 << C, moduli, pb.LaunchOpts(variant=variant))
+        totals.add(tuple(pb.pairings_sum_rows(rows, moduli)))
+    assert len(totals) == 1
+    assert pb.pairings_reconstruct(kind, n, moduli, list(totals.pop())) == (455936, 227968)
+
+
+def test_degenerate_geometries_generic():
+    # one term per chunk (C = B), n = 2, single modulus, 16 moduli
+    for kind, n in ((S, 2), (L, 2), (S, 4), (L, 3)):
+        B = 2 * n - 1
+        moduli = pb.pairings_default_moduli(2)
+        rows = gpu_rows(kind, n, B, 0, 1 << B, moduli, pb.LaunchOpts(variant=pb.VARIANT_GENERIC))
+        for c in range(1 << B):
+            assert rows[c] == oracle.chunk(kind, n, B, c, moduli)[2]
+    m16 = pb.pairings_default_moduli(16)
+    rows = gpu_rows(S, 8, 5, 0, 32, m16)
+    for c in (0, 7, 31):
+        assert rows[c] == oracle.chunk(S, 8, 5, c, m16)[2]
+    rows = gpu_rows(S, 8, 5, 3, 9, m16[:1])
+    for i, c in enumerate(range(3, 9)):
+        assert rows[i] == oracle.chunk(S, 8, 5, c, m16[:1])[2]
+
+
+def test_maximum_n_32_single_terms():
+    # n = 32: N = 64 positions, 63 index bits.  C = B makes every chunk a single sign vector, so the
+    # oracle evaluates them one by one (products up to ~2^177: exercises the full product chain).
+    moduli = pb.pairings_default_moduli(8)
+    for kind in (S, L):
+        n, B = 32, 63
+        for begin in (0, (1 << 63) - 64, 0x5DEECE66D << 20):
+            rows = gpu_rows(kind, n, B, begin, begin + 64, moduli, pb.LaunchOpts(variant=pb.VARIANT_GENERIC))
+            for i in range(0, 64, 7):
+                assert rows[i] == oracle.chunk(kind, n, B, begin + i, moduli)[2]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("kind", [S, L])
+def test_config3_n16_sampled_chunks_and_total(kind, variant, paper_counts):
+    # BASELINE config 3: 2^31 sign vectors, 5 primes + 1 check prime.
+    n, moduli = 16, pb.pairings_default_moduli(6)
+    if not variant_available(variant, kind, n, 16):
+        pytest.skip("variant not compiled")
+    C = 16
+    chunks = seeds.sample_chunks(C, 16, salt=kind)
+    want = oracle_rows(kind, n, C, chunks, moduli)            # 16 x 2^15 terms
+    for c, w in zip(chunks, want):
+        assert gpu_rows(kind, n, C, c, c + 1, moduli, pb.LaunchOpts(variant=variant))[0] == w[2], c
+    if variant == pb.VARIANT_GENERIC and kind == L:
+        # the stated geometry: 10 high bits as thread prefix, 21 Gray-code bits per thread (D3)
+        rows = gpu_rows(kind, n, 0, 0, 1, moduli, pb.LaunchOpts(variant=variant, gray_bits=21, block_threads=32, blocks_per_chunk=32))
+    else:
+        rows = gpu_rows(kind, n, 10, 0, 1 << 10, moduli, pb.LaunchOpts(variant=variant))
+    D, Sid = pb.pairings_reconstruct(kind, n, moduli, pb.pairings_sum_rows(rows, moduli))
+    assert Sid == paper_counts[(kind, n)] and D == 2 * Sid    # 700,078,384 / 326,721,800
+
+
+def test_host_buffer_call_and_run_driver_with_journal(tmp_path):
+    kind, n, C = L, 12, 8
+    moduli = pb.pairings_default_moduli(4)
+    rows = pb.count_pairings_host(kind, n, C, 10, 20, moduli)
+    assert rows == gpu_rows(kind, n, C, 10, 20, moduli)
+    path = str(tmp_path / "journal.txt")
+    total, done = pb.pairings_run(kind, n, C, moduli, 48, path, max_calls=2)       # interrupted run
+    assert done == 96
+    ranges, jt = pb.pairings_journal_load(path, kind, n, C, moduli)
+    assert ranges == [(0, 48), (48, 96)] and jt == total
+    total, done = pb.pairings_run(kind, n, C, moduli, 100, path)                  # resumed
+    assert done == 256
+    assert pb.pairings_reconstruct(kind, n, moduli, total) == (216288, 108144)
+    total2, done2 = pb.pairings_run(kind, n, C, moduli, 256, path)                # nothing left to do
+    assert (total2, done2) == (total, 256)
+    assert pb.count(S, 13) == (3040560, 1520280)                                 # config 2, both conventions
