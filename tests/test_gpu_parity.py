@@ -77,7 +77,7 @@ def test_small_n_totals_match_backtracking(kind, n, variant, paper_counts):
     C = max(0, min(5, 2 * n - 1 - 4))
     if not variant_available(variant, kind, n, C):
         pytest.skip("variant not compiled for this (kind, n)")
-    moduli = pb.pairings_default_moduli(3)
+    moduli = pb.pairings_default_moduli(pb.pairings_min_moduli(kind, n) + 1)
     rows = gpu_rows(kind, n, C, 0, 1 << C, moduli, pb.LaunchOpts(variant=variant))
     D, Sid = pb.pairings_reconstruct(kind, n, moduli, pb.pairings_sum_rows(rows, moduli))
     assert D == oracle.brute_count(kind, n)
