@@ -23,8 +23,24 @@ ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 CFLAGS = ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-I", INCLUDE, "-I", CSRC]
 
 
+def swar_instances():
+    """(kind, n) pairs of csrc/swar_list.h — swar_inst.cu is compiled once per pair."""
+    import re
+    text = open(os.path.join(CSRC, "swar_list.h")).read()
+    text = re.sub(r"//.*", "", text)
+    return [(int(k), int(n)) for k, n in re.findall(r"X\(\s*(\d+)\s*,\s*(\d+)\s*\)", text)]
+
+
 def sources():
-    return sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp")))
+    """[(source, extra defines, object tag)]"""
+    out = []
+    for f in sorted(glob.glob(os.path.join(CSRC, "*.cu")) + glob.glob(os.path.join(CSRC, "*.cpp"))):
+        if os.path.basename(f) == "swar_inst.cu":
+            for k, n in swar_instances():
+                out.append((f, ["-DPAIRINGS_SWAR_KIND=%d" % k, "-DPAIRINGS_SWAR_N=%d" % n], "_%d_%d" % (k, n)))
+        else:
+            out.append((f, [], ""))
+    return out
 
 
 def _deps_stamp():
@@ -35,11 +51,12 @@ def _deps_stamp():
     return h.hexdigest()[:16]
 
 
-def _compile(src, stamp, verbose):
-    obj = os.path.join(OBJ, os.path.basename(src) + "." + stamp + ".o")
+def _compile(item, stamp, verbose):
+    src, defines, tag = item
+    obj = os.path.join(OBJ, os.path.basename(src) + tag + "." + stamp + ".o")
     if os.path.exists(obj) and os.path.getmtime(obj) >= os.path.getmtime(src):
         return obj
-    cmd = [NVCC] + ARCH + CFLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-c", src, "-o", obj]
+    cmd = [NVCC] + ARCH + CFLAGS + (["-Xptxas", "-v"] if verbose else []) + defines + ["-c", src, "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (src, r.stdout, r.stderr))

@@ -13,6 +13,7 @@
 // every (kind, n) they are not compiled for and an independent second implementation of the rows.
 #include "pairings.h"
 #include "internal.h"
+#include "device_common.cuh"
 
 #include <cuda_runtime.h>
 
@@ -44,16 +45,8 @@ static MontPrime make_prime(uint32_t p) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// device helpers
+// device helpers (montmul, atomic_add_mod, block_reduce_write: device_common.cuh)
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t montmul(uint32_t a, uint32_t b, uint32_t p, uint32_t pinv_neg) {
-    // a*b < p*2^32  ->  returns a*b*2^{-32} mod p in [0,p)
-    const uint64_t t = (uint64_t)a * b;
-    const uint32_t m = (uint32_t)t * pinv_neg;
-    const uint32_t u = (uint32_t)((t + (uint64_t)m * p) >> 32);   // < 2p < 2^32
-    return u >= p ? u - p : u;
-}
-
 // Montgomery form (value * 2^32 mod p) of a signed 64-bit integer with |g| < 2^62
 __device__ __forceinline__ uint32_t to_mont64(long long g, const MontPrime& mp) {
     const bool neg = g < 0;
@@ -62,41 +55,6 @@ __device__ __forceinline__ uint32_t to_mont64(long long g, const MontPrime& mp) 
     if (r >= mp.p) r -= mp.p;
     if (neg && r) r = mp.p - r;
     return r;
-}
-
-// out[idx] = (out[idx] + v) mod p, atomically (several blocks may share one chunk row)
-__device__ __forceinline__ void atomic_add_mod(uint32_t* addr, uint32_t v, uint32_t p) {
-    uint32_t old = *addr, assumed;
-    do {
-        assumed = old;
-        uint32_t s = assumed + v; if (s >= p) s -= p;
-        old = atomicCAS(addr, assumed, s);
-    } while (old != assumed);
-}
-
-// Block-level sum of per-thread residues (Montgomery or plain, already < p) and the row write.
-// vals[i] < p_i.  red: shared scratch of (blockDim/32) * PAIRINGS_MAX_MODULI uint64.
-__device__ __forceinline__ void block_reduce_write(const KernelParams& kp, const uint32_t* vals,
-                                                   unsigned long long nz, unsigned long long* red,
-                                                   uint64_t chunk_local) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    for (int i = 0; i < kp.n_moduli; i++) {
-        unsigned long long v = vals[i];
-        for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-        if (lane == 0) red[warp * PAIRINGS_MAX_MODULI + i] = v;
-    }
-    for (int o = 16; o > 0; o >>= 1) nz += __shfl_xor_sync(0xffffffffu, nz, o);
-    if (lane == 0 && kp.nonzero && nz) atomicAdd(kp.nonzero, nz);
-    __syncthreads();
-    if ((int)threadIdx.x < kp.n_moduli) {
-        const int i = threadIdx.x;
-        unsigned long long s = 0;
-        for (int w = 0; w < nwarps; w++) s += red[w * PAIRINGS_MAX_MODULI + i];
-        const uint32_t p = kp.primes[i].p;
-        const uint32_t r = (uint32_t)(s % p);
-        uint32_t* dst = kp.out + chunk_local * (uint64_t)kp.n_moduli + (uint64_t)i;
-        if (kp.log2_bpc == 0) *dst = r; else atomic_add_mod(dst, r, p);
-    }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -200,42 +158,59 @@ struct Geometry { int variant, g, threads, log2_bpc; };
 
 static int choose_geometry(int kind, int n, int chunk_bits, uint64_t n_chunks,
                            const pairings_launch_opts* o, Geometry* out) {
-    const int tb = 2 * n - 1 - chunk_bits;
+    const int tb = 2 * n - 1 - chunk_bits;               // index bits inside one chunk
     int variant = o ? o->variant : PAIRINGS_VARIANT_AUTO;
     if (variant < 0 || variant > PAIRINGS_VARIANT_SWAR) return PAIRINGS_EINVAL_OPTS;
-    const int h = swar_min_gray_bits();
-    const bool swar_ok = swar_lookup(kind, n) != nullptr && tb >= h && n - 2 >= h;
-    if (variant == PAIRINGS_VARIANT_SWAR && !swar_ok) return PAIRINGS_EINVAL_OPTS;
-    if (variant == PAIRINGS_VARIANT_AUTO) variant = swar_ok ? PAIRINGS_VARIANT_SWAR : PAIRINGS_VARIANT_GENERIC;
+    int g = o ? o->gray_bits : 0, threads = o ? o->block_threads : 0, bpc = o ? o->blocks_per_chunk : 0;
+    if (g < 0 || threads < 0 || bpc < 0) return PAIRINGS_EINVAL_OPTS;
+    if (threads != 0 && (threads < 32 || threads > 256 || threads % 32)) return PAIRINGS_EINVAL_OPTS;
+    if (bpc != 0 && (!is_pow2((uint64_t)bpc) || bpc > (1 << 20))) return PAIRINGS_EINVAL_OPTS;
+    const int total_bits = tb + ilog2_floor(std::max<uint64_t>(n_chunks, 1));
 
-    const int gmin = variant == PAIRINGS_VARIANT_SWAR ? h : 0;
-    const int gmax = variant == PAIRINGS_VARIANT_SWAR ? std::min(tb, n - 2) : std::min(tb, 40);
-    int g = o ? o->gray_bits : 0;
-    if (g != 0) { if (g < gmin || g > gmax) return PAIRINGS_EINVAL_OPTS; }
-    else {
-        // default: enough thread prefixes to fill 148 SMs x 2048 threads a few times over, but at
-        // least 2^10 terms per prefix when the problem is big enough to afford it.
-        const int total_bits = tb + ilog2_floor(std::max<uint64_t>(n_chunks, 1));
-        g = total_bits - 20;
-        g = std::max(g, gmin); g = std::min(g, std::min(gmax, variant == PAIRINGS_VARIANT_SWAR ? 14 : 12));
-        g = std::max(g, gmin);
+    // ---- SWAR: whole warps of prefixes per block, every left neighbour of a walked bit exists
+    // (g <= n-2), power-of-two threads, at most 2^32 steps per thread (accumulator width).
+    const int h = swar_min_gray_bits();
+    const int swar_gmax = std::min(std::min(n - 2, 24), tb - 5);
+    bool swar_ok = swar_lookup(kind, n) != nullptr && swar_gmax >= h;
+    if (swar_ok && g != 0 && (g < h || g > swar_gmax)) swar_ok = false;
+    if (swar_ok && threads != 0 && !is_pow2((uint64_t)threads)) swar_ok = false;
+    if (swar_ok) {
+        int sg = g ? g : std::max(h, std::min(total_bits - 19, std::min(swar_gmax, 14)));
+        const int pb = tb - sg;                           // log2(prefixes per chunk) >= 5
+        int st = threads ? threads : std::min(256, 1 << std::min(pb, 8));
+        int sb = bpc;
+        if (sb == 0) {
+            sb = 1;
+            const uint64_t want_blocks = 148ULL * 8;
+            while (n_chunks * (uint64_t)sb < want_blocks && pb - ilog2_floor((uint64_t)sb) - 1 >= ilog2_floor((uint64_t)st) && sb < (1 << 20)) sb *= 2;
+            while (tb - ilog2_floor((uint64_t)sb) - ilog2_floor((uint64_t)st) > 32 && sb < (1 << 20)) sb *= 2;
+        }
+        const int lb = ilog2_floor((uint64_t)sb);
+        if (pb - lb < ilog2_floor((uint64_t)st) || tb - lb - ilog2_floor((uint64_t)st) > 32) swar_ok = false;
+        else if (variant != PAIRINGS_VARIANT_GENERIC) {
+            out->variant = PAIRINGS_VARIANT_SWAR; out->g = sg; out->threads = st; out->log2_bpc = lb;
+            return PAIRINGS_OK;
+        }
     }
-    int threads = o ? o->block_threads : 0;
-    if (threads != 0) { if (threads < 32 || threads > 256 || threads % 32) return PAIRINGS_EINVAL_OPTS; }
-    else {
+    if (variant == PAIRINGS_VARIANT_SWAR) return PAIRINGS_EINVAL_OPTS;
+
+    // ---- generic
+    const int gmax = std::min(tb, 40);
+    if (g != 0) { if (g > gmax) return PAIRINGS_EINVAL_OPTS; }
+    else g = std::max(0, std::min(total_bits - 20, std::min(gmax, 12)));
+    if (threads == 0) {
         threads = 256;
-        const int pb = tb - g;                           // log2(prefixes per chunk)
+        const int pb = tb - g;
         if (pb < 8) threads = std::max(32, 1 << pb);
     }
-    int bpc = o ? o->blocks_per_chunk : 0;
     const uint64_t prefixes = 1ULL << std::min(tb - g, 62);
-    if (bpc != 0) { if (!is_pow2((uint64_t)bpc) || (uint64_t)bpc > prefixes || bpc > (1 << 20)) return PAIRINGS_EINVAL_OPTS; }
+    if (bpc != 0) { if ((uint64_t)bpc > prefixes) return PAIRINGS_EINVAL_OPTS; }
     else {
         bpc = 1;
-        const uint64_t want_blocks = 148ULL * 16;        // a few waves
+        const uint64_t want_blocks = 148ULL * 16;
         while (n_chunks * (uint64_t)bpc < want_blocks && (uint64_t)bpc * 2 * (uint64_t)threads <= prefixes && bpc < (1 << 20)) bpc *= 2;
     }
-    out->variant = variant; out->g = g; out->threads = threads; out->log2_bpc = ilog2_floor((uint64_t)bpc);
+    out->variant = PAIRINGS_VARIANT_GENERIC; out->g = g; out->threads = threads; out->log2_bpc = ilog2_floor((uint64_t)bpc);
     return PAIRINGS_OK;
 }
 

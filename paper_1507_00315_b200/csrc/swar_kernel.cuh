@@ -1,0 +1,486 @@
+// SWAR Gray-code kernel, specialised per (kind, n) — the fast path of count_pairings.
+//
+// What it computes is exactly §8(a) rows a2..a6 (PAPER.md:176 Gray-code ordering, PAPER.md:257
+// residues modulo co-primes); how it computes it is designed for sm_100a's integer pipes:
+//
+//  * pair-sums live byte-packed, four per 32-bit register ("slots"): slot value = Q_k + 128 with
+//    Q_k = P_k/2 for even d_k (P_k = N-d_k mod 2, so these are the only sums that can vanish) and
+//    Q_k = P_k for odd d_k.  The factor 2^{#even} is restored once per thread at the end.
+//    Even-d slots come first, so the zero test (row a4) looks at NT = ceil(#even/4) registers:
+//    a byte is 0x80 iff  bit7(v) & ~bit7(v - 0x01010101).
+//  * the low H = 4 index bits are walked by two fully unrolled 16-step Gray blocks (block parity =
+//    state of inner bit 3).  For every inner position the packed vector C[b] of its neighbours that
+//    lie OUTSIDE the inner bits is kept in registers; neighbours inside the inner bits are known at
+//    compile time and folded into an immediate.  One Gray step (row a3) is therefore
+//         Q[r] = Q[r] -/+ C[b][r] + K[r]          — one 3-input add per register, n/4 per step,
+//    instead of n boundary-guarded updates.  (Deltas are added as whole 32-bit integers: bytes stay
+//    in [65,191] after every step, so no carry ever crosses a slot.)
+//  * index bits H..g-1 ("outer" flips, once per 16 steps) rebuild the neighbour vector of the
+//    flipped position from two de-interleaved copies (E: even index bits, O: odd) of the sign word
+//    with a multiply-spread (4 bits -> 4 bytes), and patch one byte of each C[b].
+//    Because g <= n-2, every left neighbour of a walked position exists: no boundary guards at all.
+//  * non-zero terms are compacted (row a4's divergence problem): ballot + popc prefix push the packed
+//    registers + sign into a per-warp shared-memory ring; whenever 32 entries are queued all lanes
+//    multiply one entry each (any lane may process any term of its warp: the sum is commutative and
+//    a warp never spans two chunks).
+//  * row a5: the product is formed as G exact signed group products (< 2^31 each), multiplied to a
+//    multi-word magnitude and added, with sign, into a W-word two's-complement accumulator.  The
+//    reduction modulo the primes happens ONCE per thread (32-bit Montgomery Horner), not per term —
+//    the residues written are identical, the per-term cost no longer depends on the number of primes.
+//  * row a6: shared with the generic kernel (block_reduce_write).
+#pragma once
+
+#include "internal.h"
+#include "device_common.cuh"
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <type_traits>
+
+namespace pairings {
+namespace swar {
+
+constexpr int H = 4;              // unrolled inner Gray bits
+constexpr int BLK = 1 << H;       // steps per unrolled block
+constexpr int QCAP = 256;         // ring entries per warp (power of two)
+constexpr int CHECK_EVERY = 4;    // steps between drain checks; 31 + 32*CHECK_EVERY < QCAP
+
+#define PAIRINGS_HD __host__ __device__ constexpr
+
+// compile-time loop: f(std::integral_constant<int, I>) for I in [I0, I1)
+template <int I0, int I1, class F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (I0 < I1) {
+        f(std::integral_constant<int, I0>{});
+        static_for<I0 + 1, I1>(f);
+    }
+}
+#define PAIRINGS_IC(name, ic) constexpr int name = decltype(ic)::value
+
+PAIRINGS_HD int ctz_c(int v) { int c = 0; while (((v >> c) & 1) == 0) c++; return c; }
+PAIRINGS_HD int gray_c(int s) { return s ^ (s >> 1); }
+PAIRINGS_HD int bitlen_c(uint64_t v) { int c = 0; while (v) { c++; v >>= 1; } return c; }
+
+// ------------------------------------------------------------------------------------------------
+// compile-time layout of one (kind, n)
+// ------------------------------------------------------------------------------------------------
+template <int KIND, int NN>
+struct Lay {
+    static constexpr int N = 2 * NN;
+    PAIRINGS_HD static int d_of_k(int k) { return KIND == PAIRINGS_SKOLEM ? k : k + 1; }
+    PAIRINGS_HD static int n_even() { int c = 0; for (int k = 1; k <= NN; k++) c += (d_of_k(k) % 2 == 0); return c; }
+    // slot order: even distances ascending, then odd distances ascending
+    PAIRINGS_HD static int d_of_slot(int s) {
+        int c = 0;
+        for (int k = 1; k <= NN; k++) if (d_of_k(k) % 2 == 0) { if (c == s) return d_of_k(k); c++; }
+        for (int k = 1; k <= NN; k++) if (d_of_k(k) % 2 == 1) { if (c == s) return d_of_k(k); c++; }
+        return 0;
+    }
+    PAIRINGS_HD static int slot_of_d(int d) { for (int s = 0; s < NN; s++) if (d_of_slot(s) == d) return s; return -1; }
+    PAIRINGS_HD static int unit(int s) { return d_of_slot(s) % 2 == 0 ? 1 : 2; }      // |dQ| per neighbour product
+    PAIRINGS_HD static int cnt(int s) { return N - d_of_slot(s); }                     // number of summands of P
+    PAIRINGS_HD static int bound(int s) { return d_of_slot(s) % 2 == 0 ? cnt(s) / 2 : cnt(s); }   // |Q| <= bound
+    static constexpr int NR = (NN + 3) / 4;            // packed registers
+    static constexpr int NT = (n_even() + 3) / 4;      // registers that need the zero test
+    // greedy grouping of slots into exact signed 32-bit products
+    PAIRINGS_HD static int group_of_slot(int s) {
+        int g = 0; uint64_t prod = 1;
+        for (int t = 0; t <= s; t++) {
+            if (prod * (uint64_t)bound(t) >= (1ULL << 31)) { g++; prod = 1; }
+            prod *= (uint64_t)bound(t);
+        }
+        return g;
+    }
+    PAIRINGS_HD static int n_groups() { return group_of_slot(NN - 1) + 1; }
+    PAIRINGS_HD static int term_bits() {                // upper bound on bitlen(|prod_k Q_k|)
+        int bits = 0, g = 0; uint64_t prod = 1;
+        for (int t = 0; t < NN; t++) {
+            if (group_of_slot(t) != g) { bits += bitlen_c(prod); prod = 1; g = group_of_slot(t); }
+            prod *= (uint64_t)bound(t);
+        }
+        return bits + bitlen_c(prod);
+    }
+    static constexpr int G = n_groups();
+    // accumulator words: |sum| < 2^term_bits * 2^32 drained terms per thread (host enforces), + sign
+    static constexpr int W = (term_bits() + 33 + 31) / 32;
+    static_assert(W >= G && W <= 8, "accumulator must hold the multi-word product");
+    static constexpr int EW = NR + 1;                   // ring entry words (packed sums + sign)
+    static constexpr uint32_t PAD = 0x40;               // value of unused slots (never reads as zero)
+};
+
+// ------------------------------------------------------------------------------------------------
+// neighbour vectors
+// ------------------------------------------------------------------------------------------------
+// Byte-spread of the low L <= 4 bits of x: bit i -> bit 8i.
+__device__ __forceinline__ uint32_t spread4(uint32_t x) { return (x * 0x00204081u) & 0x01010101u; }
+
+// left_vec<b, INNER>: packed vector over slots of  unit(s) * x_{bit b + d_s}  (the LEFT neighbour of
+// index bit b at distance d_s; it always exists for b <= n-3), as a 32-bit integer per register:
+//     out[r] = sum_{s in r} unit(s) * x * 256^{s%4}      (signed bytes added as integers).
+// INNER: only neighbours outside the inner bits (b + d_s >= H) are included.
+// !INNER: the RIGHT neighbours (index bit b - d_s >= 0) are added too; at the moment bit b flips in
+//         Gray order bit b-1 is 1 and all lower bits are 0, so they are compile-time constants.
+template <int KIND, int NN, int b, bool INNER>
+struct LeftVec {
+    using L = Lay<KIND, NN>;
+    // is slot s included, and does it start a run of slots whose neighbours are consecutive bits of E or O
+    PAIRINGS_HD static bool included(int s) { return s < NN && !(INNER && b + L::d_of_slot(s) < H); }
+    PAIRINGS_HD static bool run_start(int s) {
+        if (!included(s)) return false;
+        if (s % 4 == 0) return true;
+        return !(included(s - 1) && L::d_of_slot(s - 1) == L::d_of_slot(s) - 2);
+    }
+    PAIRINGS_HD static int run_len(int s) {
+        int len = 1;
+        while ((s + len) % 4 != 0 && included(s + len) && L::d_of_slot(s + len) == L::d_of_slot(s) + 2 * len) len++;
+        return len;
+    }
+    PAIRINGS_HD static uint32_t base(int r) {
+        uint32_t v = 0;
+        for (int o = 0; o < 4; o++) {
+            const int s = 4 * r + o;
+            if (s >= NN) continue;
+            const int d = L::d_of_slot(s), u = L::unit(s);
+            if (!INNER && d <= b) v += (uint32_t)(d == 1 ? -u : u) << (8 * o);   // right neighbour, known
+            if (included(s)) v += (uint32_t)u << (8 * o);                          // x = +1 part of the left neighbour
+        }
+        return v;
+    }
+    __device__ __forceinline__ static void eval(uint32_t E, uint32_t O, uint32_t (&out)[L::NR]) {
+        static_for<0, L::NR>([&](auto rc) {
+            PAIRINGS_IC(r, rc);
+            uint32_t var = 0;
+            static_for<0, 4>([&](auto oc) {
+                PAIRINGS_IC(o, oc);
+                constexpr int s = 4 * r + o;
+                if constexpr (run_start(s)) {
+                    constexpr int d = L::d_of_slot(s), u = L::unit(s), len = run_len(s);
+                    const uint32_t word = ((b + d) & 1) ? O : E;
+                    const uint32_t bits = (word >> ((b + d) >> 1)) & ((1u << len) - 1u);
+                    var += spread4(bits) * (uint32_t)((2 * u) << (8 * o));       // a run shares the parity of d, hence the unit
+                }
+            });
+            constexpr uint32_t bs = base(r);
+            out[r] = bs - var;
+        });
+    }
+};
+
+// ------------------------------------------------------------------------------------------------
+// compile-time constants of the unrolled inner blocks
+// ------------------------------------------------------------------------------------------------
+// inner state (bit set <-> x = -1) at inner step S of a block with parity PAR
+PAIRINGS_HD int zbits(int par, int s) { return gray_c(s) ^ (par << (H - 1)); }
+
+// K: contribution of the inner neighbours to dQ when inner bit bi = ctz(S+1) flips at step S -> S+1
+template <int KIND, int NN>
+PAIRINGS_HD uint32_t kconst(int par, int S, int r) {
+    using L = Lay<KIND, NN>;
+    const int zb = zbits(par, S), bi = ctz_c(S + 1);
+    const int xo = 1 - 2 * ((zb >> bi) & 1);
+    uint32_t K = 0;
+    for (int o = 0; o < 4; o++) {
+        const int s = 4 * r + o;
+        if (s >= NN) continue;
+        const int d = L::d_of_slot(s), u = L::unit(s);
+        int nb = 0;
+        if (bi + d < H) nb += 1 - 2 * ((zb >> (bi + d)) & 1);     // inner left neighbour
+        if (bi - d >= 0) nb += 1 - 2 * ((zb >> (bi - d)) & 1);    // right neighbour (always inner)
+        K += (uint32_t)(-u * xo * nb) << (8 * o);
+    }
+    return K;
+}
+
+// ------------------------------------------------------------------------------------------------
+// ring entry -> signed multi-word term -> accumulator
+// ------------------------------------------------------------------------------------------------
+template <int W>
+__device__ __forceinline__ void acc_add_signed(uint32_t (&acc)[W], const uint32_t* x /* W words, already ^mask */, uint32_t mask) {
+    // acc += x + (mask & 1)  with carry propagation (two's complement add of +-T)
+    uint32_t dummy;
+    static_assert(W >= 2 && W <= 8, "accumulator width");
+    if constexpr (W == 2) {
+        asm volatile("add.cc.u32 %2, %5, 1;\n\taddc.cc.u32 %0, %0, %3;\n\taddc.u32 %1, %1, %4;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "=r"(dummy) : "r"(x[0]), "r"(x[1]), "r"(mask));
+    } else if constexpr (W == 3) {
+        asm volatile("add.cc.u32 %3, %7, 1;\n\taddc.cc.u32 %0, %0, %4;\n\taddc.cc.u32 %1, %1, %5;\n\taddc.u32 %2, %2, %6;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "=r"(dummy) : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(mask));
+    } else if constexpr (W == 4) {
+        asm volatile("add.cc.u32 %4, %9, 1;\n\taddc.cc.u32 %0, %0, %5;\n\taddc.cc.u32 %1, %1, %6;\n\taddc.cc.u32 %2, %2, %7;\n\taddc.u32 %3, %3, %8;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "=r"(dummy)
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(mask));
+    } else if constexpr (W == 5) {
+        asm volatile("add.cc.u32 %5, %11, 1;\n\taddc.cc.u32 %0, %0, %6;\n\taddc.cc.u32 %1, %1, %7;\n\taddc.cc.u32 %2, %2, %8;\n\t"
+                     "addc.cc.u32 %3, %3, %9;\n\taddc.u32 %4, %4, %10;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "=r"(dummy)
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(mask));
+    } else if constexpr (W == 6) {
+        asm volatile("add.cc.u32 %6, %13, 1;\n\taddc.cc.u32 %0, %0, %7;\n\taddc.cc.u32 %1, %1, %8;\n\taddc.cc.u32 %2, %2, %9;\n\t"
+                     "addc.cc.u32 %3, %3, %10;\n\taddc.cc.u32 %4, %4, %11;\n\taddc.u32 %5, %5, %12;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "+r"(acc[5]), "=r"(dummy)
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(mask));
+    } else if constexpr (W == 7) {
+        asm volatile("add.cc.u32 %7, %15, 1;\n\taddc.cc.u32 %0, %0, %8;\n\taddc.cc.u32 %1, %1, %9;\n\taddc.cc.u32 %2, %2, %10;\n\t"
+                     "addc.cc.u32 %3, %3, %11;\n\taddc.cc.u32 %4, %4, %12;\n\taddc.cc.u32 %5, %5, %13;\n\taddc.u32 %6, %6, %14;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "+r"(acc[5]), "+r"(acc[6]), "=r"(dummy)
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(mask));
+    } else {
+        asm volatile("add.cc.u32 %8, %17, 1;\n\taddc.cc.u32 %0, %0, %9;\n\taddc.cc.u32 %1, %1, %10;\n\taddc.cc.u32 %2, %2, %11;\n\t"
+                     "addc.cc.u32 %3, %3, %12;\n\taddc.cc.u32 %4, %4, %13;\n\taddc.cc.u32 %5, %5, %14;\n\taddc.cc.u32 %6, %6, %15;\n\t"
+                     "addc.u32 %7, %7, %16;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "+r"(acc[5]), "+r"(acc[6]), "+r"(acc[7]), "=r"(dummy)
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(x[7]), "r"(mask));
+    }
+}
+
+template <int KIND, int NN>
+__device__ __forceinline__ void drain_entry(const uint32_t* __restrict__ ring, uint32_t idx,
+                                            uint32_t (&acc)[Lay<KIND, NN>::W]) {
+    using L = Lay<KIND, NN>;
+    constexpr int NR = L::NR, G = L::G, W = L::W;
+    uint32_t w[NR];
+#pragma unroll
+    for (int r = 0; r < NR; r++) w[r] = ring[r * QCAP + idx] ^ 0x80808080u;      // bytes -> two's complement Q
+    int gp[G];
+#pragma unroll
+    for (int g = 0; g < G; g++) gp[g] = 1;
+    gp[0] = (int)ring[NR * QCAP + idx];                                           // sign of the term
+    static_for<0, NN>([&](auto sc) {
+        PAIRINGS_IC(s, sc);
+        const int q = (int)(int8_t)(w[s / 4] >> (8 * (s % 4)));
+        constexpr int g = L::group_of_slot(s);
+        gp[g] *= q;                                                               // exact: |group| < 2^31
+    });
+    // sign-magnitude: multi-word product of |gp[i]|
+    uint32_t sx = 0;
+#pragma unroll
+    for (int g = 0; g < G; g++) sx ^= (uint32_t)gp[g];
+    const uint32_t mask = (uint32_t)((int)sx >> 31);                              // all ones iff the term is negative
+    uint32_t T[W];
+#pragma unroll
+    for (int i = 0; i < W; i++) T[i] = 0;
+    T[0] = (uint32_t)abs(gp[0]);
+#pragma unroll
+    for (int g = 1; g < G; g++) {
+        const uint32_t m = (uint32_t)abs(gp[g]);
+        uint32_t carry = 0;
+#pragma unroll
+        for (int i = 0; i < g; i++) {
+            const uint64_t p = (uint64_t)T[i] * m + carry;
+            T[i] = (uint32_t)p; carry = (uint32_t)(p >> 32);
+        }
+        T[g] = carry;
+    }
+#pragma unroll
+    for (int i = 0; i < W; i++) T[i] ^= mask;
+    acc_add_signed<W>(acc, T, mask);
+}
+
+// ------------------------------------------------------------------------------------------------
+// the kernel
+// ------------------------------------------------------------------------------------------------
+template <int KIND, int NN>
+struct Walker {
+    using L = Lay<KIND, NN>;
+    static constexpr int NR = L::NR, NT = L::NT, W = L::W, EW = L::EW;
+
+    uint32_t Q[NR];
+    uint32_t C[H][NR];
+    uint32_t E, O;            // de-interleaved sign word: E bit i = index bit 2i, O bit i = index bit 2i+1
+    uint32_t acc[W];
+    uint32_t tail, head;      // warp-uniform ring counters (monotone)
+    uint32_t sgn_even, sgn_odd;   // sign word pushed at even / odd inner steps (+1 / -1 as int)
+    uint32_t ltmask;
+    uint32_t* ring;
+    int lane;
+
+    __device__ __forceinline__ void push_if_nonzero(uint32_t sgnword) {
+        uint32_t z = 0;
+#pragma unroll
+        for (int r = 0; r < NT; r++) z |= Q[r] & ~(Q[r] - 0x01010101u);
+        const bool nonzero = (z & 0x80808080u) == 0;
+        const uint32_t bal = __ballot_sync(0xffffffffu, nonzero);
+        if (nonzero) {
+            const uint32_t idx = (tail + __popc(bal & ltmask)) & (QCAP - 1);
+#pragma unroll
+            for (int r = 0; r < NR; r++) ring[r * QCAP + idx] = Q[r];
+            ring[NR * QCAP + idx] = sgnword;
+        }
+        tail += __popc(bal);
+    }
+
+    __device__ __forceinline__ void drain_full() {
+        while (tail - head >= 32u) {
+            __syncwarp();
+            drain_entry<KIND, NN>(ring, (head + (uint32_t)lane) & (QCAP - 1), acc);
+            head += 32u;
+            __syncwarp();
+        }
+    }
+
+    __device__ __forceinline__ void drain_rest() {
+        drain_full();
+        __syncwarp();
+        if ((uint32_t)lane < tail - head) drain_entry<KIND, NN>(ring, (head + (uint32_t)lane) & (QCAP - 1), acc);
+        head = tail;
+        __syncwarp();
+    }
+
+    template <int PAR, int S>
+    __device__ __forceinline__ void inner_steps() {
+        if constexpr (S < BLK) {
+            push_if_nonzero((S & 1) ? sgn_odd : sgn_even);
+            if constexpr ((S + 1) % CHECK_EVERY == 0) drain_full();
+            if constexpr (S + 1 < BLK) {
+                constexpr int bi = ctz_c(S + 1);
+                constexpr int xo = 1 - 2 * ((zbits(PAR, S) >> bi) & 1);              // old x_j
+                static_for<0, NR>([&](auto rc) {
+                    PAIRINGS_IC(r, rc);
+                    constexpr uint32_t K = kconst<KIND, NN>(PAR, S, r);
+                    if constexpr (xo > 0) Q[r] = Q[r] - C[bi][r] + K;                // dQ = -x_j * C + K
+                    else Q[r] = Q[r] + C[bi][r] + K;
+                });
+            }
+            inner_steps<PAR, S + 1>();
+        }
+    }
+
+    // flip of index bit b >= H (between two inner blocks)
+    template <int b>
+    __device__ __forceinline__ void outer_flip() {
+        const uint32_t word = (b & 1) ? O : E;
+        const uint32_t sg = 1u - 2u * ((word >> (b >> 1)) & 1u);       // old x_j as +-1 (mod 2^32)
+        uint32_t t[NR];
+        LeftVec<KIND, NN, b, false>::eval(E, O, t);
+        static_for<0, NR>([&](auto rc) { PAIRINGS_IC(r, rc); Q[r] -= sg * t[r]; });   // dQ = -x_j * (left + right neighbours)
+        static_for<0, H>([&](auto bc) {
+            PAIRINGS_IC(bi, bc);
+            constexpr int s = L::slot_of_d(b - bi);
+            if constexpr (s >= 0) {
+                // byte s of C[bi] holds unit * x_j and x_j changes sign: delta = -2 * unit * old x_j
+                constexpr uint32_t k = (uint32_t)((2 * L::unit(s)) << (8 * (s % 4)));
+                C[bi][s / 4] -= sg * k;
+            }
+        });
+        if (b & 1) O ^= 1u << (b >> 1); else E ^= 1u << (b >> 1);
+    }
+
+    template <int b>
+    __device__ __forceinline__ void outer_flip_dispatch(int bit) {
+        if constexpr (b <= NN - 3) {
+            if (bit == b) outer_flip<b>(); else outer_flip_dispatch<b + 1>(bit);
+        }
+    }
+
+    // direct evaluation for the prefix V (low g bits zero): Q, C[0..H), E, O  (row a2)
+    __device__ __forceinline__ void init_prefix(uint64_t V) {
+        static_for<0, NR>([&](auto rc) {
+            PAIRINGS_IC(r, rc);
+            uint32_t q = 0;
+            static_for<0, 4>([&](auto oc) {
+                PAIRINGS_IC(o, oc);
+                constexpr int s = 4 * r + o;
+                if constexpr (s >= NN) { q |= L::PAD << (8 * o); }
+                else {
+                    constexpr int d = L::d_of_slot(s), c = L::cnt(s);
+                    const int pc = __popcll((V ^ (V >> d)) & ((1ULL << c) - 1ULL));
+                    const int qv = (L::unit(s) == 1) ? (c / 2 - pc) : (c - 2 * pc);
+                    q |= (uint32_t)(qv + 128) << (8 * o);
+                }
+            });
+            Q[r] = q;
+        });
+        uint32_t e = 0, o = 0;                                          // de-interleave
+#pragma unroll
+        for (int i = 0; i < 32; i++) {
+            e |= (uint32_t)((V >> (2 * i)) & 1ULL) << i;
+            o |= (uint32_t)((V >> (2 * i + 1)) & 1ULL) << i;
+        }
+        E = e; O = o;
+        static_for<0, H>([&](auto bc) { PAIRINGS_IC(bi, bc); LeftVec<KIND, NN, bi, true>::eval(E, O, C[bi]); });
+        const int s0 = (__popcll(V) & 1) ? -1 : 1;
+        sgn_even = (uint32_t)s0; sgn_odd = (uint32_t)(-s0);
+    }
+};
+
+template <int KIND, int NN>
+__global__ void __launch_bounds__(256)
+swar_kernel(const __grid_constant__ KernelParams kp) {
+    using L = Lay<KIND, NN>;
+    using Wk = Walker<KIND, NN>;
+    constexpr int N = L::N, B = N - 1, W = L::W;
+    extern __shared__ uint32_t smem[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
+    unsigned long long* red = reinterpret_cast<unsigned long long*>(smem);              // 8 * 16 uint64
+    uint32_t* rings = smem + 8 * PAIRINGS_MAX_MODULI * 2;
+
+    const int C = kp.chunk_bits, g = kp.gray_bits;
+    const uint64_t chunk_local = (uint64_t)blockIdx.x >> kp.log2_bpc;
+    const uint64_t sub = (uint64_t)blockIdx.x & ((1ULL << kp.log2_bpc) - 1);
+    const uint64_t chunk = kp.chunk_begin + chunk_local;
+    const int tb = B - C;
+    const uint64_t per_block = (1ULL << (tb - g)) >> kp.log2_bpc;     // multiple of blockDim (host)
+    const uint64_t chunk_base = chunk << tb;                          // tb >= H > 0
+    const uint32_t nblk = 1u << (g - H);
+
+    Wk wk;
+    wk.lane = lane;
+    wk.ltmask = (1u << lane) - 1u;
+    wk.ring = rings + (size_t)warp * (QCAP * L::EW);
+    wk.tail = 0; wk.head = 0;
+#pragma unroll
+    for (int i = 0; i < W; i++) wk.acc[i] = 0;
+    unsigned long long nz = 0;
+
+    for (uint64_t q = sub * per_block + threadIdx.x; q < (sub + 1) * per_block; q += blockDim.x) {
+        wk.init_prefix(chunk_base | (q << g));
+        const uint32_t tail0 = wk.tail;
+        for (uint32_t tout = 0; tout < nblk; tout += 2) {
+            wk.template inner_steps<0, 0>();
+            if (tout + 1 < nblk) {
+                wk.template outer_flip<H>();                           // tout+1 is odd: always bit H
+                wk.template inner_steps<1, 0>();
+                if (tout + 2 < nblk) wk.template outer_flip_dispatch<H + 1>(H + (__ffs((int)(tout + 2)) - 1));
+            }
+        }
+        nz += (unsigned long long)(wk.tail - tail0);
+    }
+    wk.drain_rest();
+    (void)nwarps;
+
+    // ---- once per thread: accumulator (W-word two's complement) -> residues, times 2^{#even}
+    uint32_t vals[PAIRINGS_MAX_MODULI];
+    const bool neg = (wk.acc[W - 1] >> 31) != 0;
+#pragma unroll 1
+    for (int i = 0; i < kp.n_moduli; i++) {
+        const MontPrime mp = kp.primes[i];
+        uint32_t r = 0;
+        uint32_t pw = mp.r1;                                           // 2^{32 j} mod p
+#pragma unroll
+        for (int j = W - 1; j >= 0; j--) {
+            r = montmul(r, mp.r2, mp.p, mp.pinv_neg) + montmul(wk.acc[j], mp.r1, mp.p, mp.pinv_neg);   // r*2^32 + acc[j]
+            if (r >= mp.p) r -= mp.p;
+        }
+#pragma unroll
+        for (int j = 1; j < W; j++) pw = montmul(pw, mp.r2, mp.p, mp.pinv_neg);                        // 2^{32 W} mod p
+        if (neg) { r = (r >= pw) ? r - pw : r + mp.p - pw; }
+        const uint32_t two_ne = montmul(1u << L::n_even(), mp.r2, mp.p, mp.pinv_neg);                  // 2^{#even} * 2^32
+        vals[i] = montmul(r, two_ne, mp.p, mp.pinv_neg);
+    }
+    // lane 0 of each warp carries the warp's non-zero count (tail is warp-uniform)
+    __syncthreads();
+    block_reduce_write(kp, vals, lane == 0 ? nz : 0ULL, red, chunk_local);
+}
+
+template <int KIND, int NN>
+int launch(const KernelParams& kp, int block_threads, unsigned grid, void* stream) {
+    using L = Lay<KIND, NN>;
+    const size_t smem = (size_t)(8 * PAIRINGS_MAX_MODULI * 2 + (block_threads / 32) * QCAP * L::EW) * sizeof(uint32_t);
+    cudaError_t e = cudaFuncSetAttribute(swar_kernel<KIND, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return (int)e;
+    swar_kernel<KIND, NN><<<grid, block_threads, smem, (cudaStream_t)stream>>>(kp);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace swar
+}  // namespace pairings

@@ -47,7 +47,7 @@ def oracle_rows(kind, n, C, chunks, moduli, threads=8):
 
 def variant_available(variant, kind, n, C):
     if variant == pb.VARIANT_SWAR:
-        return pb.pairings_has_swar(kind, n) and (2 * n - 1 - C) >= 4
+        return pb.pairings_has_swar(kind, n) and (2 * n - 1 - C) >= 9   # >= 32 prefixes of >= 2^4 steps per chunk
     return True
 
 
@@ -97,7 +97,7 @@ def test_geometry_never_changes_the_rows(variant):
     gs = [4, 7, 10] if variant == pb.VARIANT_SWAR else [0, 1, 5, 12, 17]
     for g in gs:
         for threads, bpc in ((32, 1), (128, 2), (256, 1), (64, 8)):
-            if bpc * threads > (1 << (2 * n - 1 - C - g)) and bpc > 1:
+            if bpc * threads > (1 << (2 * n - 1 - C - g)) and (bpc > 1 or variant == pb.VARIANT_SWAR):
                 continue
             o = pb.LaunchOpts(variant=variant, gray_bits=g, block_threads=threads, blocks_per_chunk=bpc)
             assert gpu_rows(kind, n, C, 0, 1 << C, moduli, o) == ref, (g, threads, bpc)
