@@ -1,0 +1,386 @@
+#!/usr/bin/env python
+"""bench.py — Godfrey sign-vector terms/s on B200 (BASELINE.json metric), one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference]
+
+A "step" is one pass of the whole hot path over the workload: partition -> count_pairings (the
+Gray-code kernel over every chunk of this rank's range) -> rows D2H -> row sums -> (rank 0, after
+the exchange of the per-rank sums) CRT + exact division, checked against the paper's printed count.
+Workload at every N: Langford L(20) — 2^39 sign vectors (x_1 = +1), 2^16 prefix chunks, 6 CRT primes
++ 1 check prime (BASELINE.json configs[3], the n = 20 point the metric is quoted on).  For N > 1 the
+2^16 chunks are dealt out as contiguous ranges (pairings_rank_range), total work fixed: "strong".
+
+`value`   = terms/s with the rows left in HBM (CUDA events around the kernel launches of a step).
+`e2e`     = terms/s through count_pairings_host (HOST output buffer; allocation, launch, D2H copy
+            and synchronise inside the timed region, wall clock).
+`roofline`= SURVEY.md §8(d) yardstick ops/term (W + phi*M, phi measured live) x terms/s against the
+            SM integer-issue peak 148 x 128 lanes x sm_max_mhz; calibration kernels measured beside it.
+`cpu_baseline` = the CPU oracle (oracle/, as it stands) on the host cores, bounded sample.
+"""
+from __future__ import annotations
+
+import argparse
+import ctypes
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+KIND_NAME = {0: "S", 1: "L"}
+# workload (BASELINE.json configs[3]): Langford n = 20, 2^16 chunks, 6 primes + 1 check prime
+WL = dict(kind=1, n=20, chunk_bits=16, n_moduli=7)
+L20_IDENTIFIED = 2636337861200          # L(20), PAPER.md:380 (Table 8)
+# secondary point of the metric (configs[4]): Skolem n = 24, 2^20 chunks, 8 primes + 1 check prime,
+# a fixed seeded 1/64 subset of chunks (256 runs of 64 contiguous chunks)
+WL24 = dict(kind=0, n=24, chunk_bits=20, n_moduli=9, runs=256, run_len=64)
+SM_COUNT, LANES_PER_SM_CLK = 148, 128
+
+
+def yardstick_ops(kind: int, n: int, n_moduli: int, phi: float):
+    """ops(kind,n,m') = W + phi*M, W = 3n+3, M = (n-G) + m'(5(G-1)+3), G = greedy
+    grouping of the factor bounds 2n-d_k into exact <= 31-bit partial products."""
+    bounds = [2 * n - (k if kind == 0 else k + 1) for k in range(1, n + 1)]
+    G, prod = 1, 1
+    for b in bounds:
+        if prod * b >= 1 << 31:
+            G, prod = G + 1, 1
+        prod *= b
+    W = 3 * n + 3
+    M = (n - G) + n_moduli * (5 * (G - 1) + 3)
+    return W + phi * M, dict(W=W, M=M, G=G, phi=phi)
+
+
+def host_threads() -> int:
+    try:
+        return max(1, len(os.sched_getaffinity(0)))
+    except AttributeError:
+        return os.cpu_count() or 1
+
+
+# ------------------------------------------------------------------------------------------------
+# CPU oracle timing (cpu_baseline leg and --impl reference)
+# ------------------------------------------------------------------------------------------------
+def oracle_sample(kind, n, sample_bits, chunks, threads):
+    """Times oracle.chunk on `chunks` (indices of the 2^sample_bits partition) with `threads` host
+    threads (ctypes releases the GIL).  Returns (terms, seconds)."""
+    import oracle
+    oracle.build()
+    moduli = []
+    todo = list(chunks)
+    lock = threading.Lock()
+
+    def work():
+        while True:
+            with lock:
+                if not todo:
+                    return
+                c = todo.pop()
+            oracle.chunk(kind, n, sample_bits, c, moduli)
+
+    t0 = time.perf_counter()
+    ts = [threading.Thread(target=work) for _ in range(threads)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    dt = time.perf_counter() - t0
+    terms = len(chunks) * (1 << (2 * n - 1 - sample_bits))
+    return terms, dt
+
+
+def cpu_baseline(kind, n, target_seconds=15.0):
+    from paper_1507_00315_b200 import seeds
+    threads = host_threads()
+    sample_bits = 2 * n - 1 - 17                       # 2^17 terms per oracle chunk
+    probe = seeds.sample_chunks(sample_bits, threads, salt=7)
+    terms, dt = oracle_sample(kind, n, sample_bits, probe, threads)
+    rate = terms / dt
+    count = int(max(threads, min(4096, target_seconds * rate / (1 << 17))))
+    chunks = seeds.sample_chunks(sample_bits, count, salt=11)
+    terms, dt = oracle_sample(kind, n, sample_bits, chunks, threads)
+    return dict(value=terms / dt, unit="terms/s", cores=threads, kind="oracle",
+                sample="%d seeded chunks of 2^17 sign vectors of %s(%d) (2^%d-chunk partition of the x_1=+1 half), "
+                       "%.1f s on %d threads" % (len(chunks), KIND_NAME[kind], n, sample_bits, dt, threads))
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores; rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_1507_00315_b200 import seeds
+    kind, n = WL["kind"], WL["n"]
+    threads = host_threads()
+    sample_bits = 2 * n - 1 - 17
+    per_step = 16 * threads
+    steps, warm = args.steps, args.warmup
+    for w in range(warm):
+        oracle_sample(kind, n, sample_bits, seeds.sample_chunks(sample_bits, threads, salt=100 + w), threads)
+    terms_total, t_total = 0, 0.0
+    for s in range(steps):
+        terms, dt = oracle_sample(kind, n, sample_bits, seeds.sample_chunks(sample_bits, per_step, salt=200 + s), threads)
+        terms_total += terms
+        t_total += dt
+    value = terms_total / t_total
+    sample = "%d seeded chunks of 2^17 sign vectors of L(20) per step on %d threads" % (per_step, threads)
+    line = dict(impl="reference", metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s",
+                n_gpus=args.gpus, steps=steps, warmup=warm, ms_per_step=1e3 * t_total / steps,
+                higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
+                config=dict(workload="L(20): Langford n=20, bounded oracle sample per step", sample=sample),
+                cpu_baseline=dict(value=value, unit="terms/s", cores=threads, kind="oracle", sample=sample),
+                e2e=dict(value=value, unit="terms/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------------------------
+# clocks
+# ------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append((time.perf_counter(), ln.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.25)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for t, ln in self.lines:
+            if t < t0 or t > t1 + 0.3:
+                continue
+            f = [x.strip() for x in ln.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx = float(f[1])
+            except (ValueError, IndexError):
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=mx, samples=len(sm), reasons=sorted(reasons))
+
+
+# ------------------------------------------------------------------------------------------------
+# GPU arm
+# ------------------------------------------------------------------------------------------------
+def run_gpu(args):
+    import torch
+    import paper_1507_00315_b200 as pb
+    from paper_1507_00315_b200 import seeds
+
+    pb.lib()                                   # fails loudly if the CUDA library is missing
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    kind, n, C, m = WL["kind"], WL["n"], WL["chunk_bits"], WL["n_moduli"]
+    moduli = pb.pairings_default_moduli(m)
+    begin, end = pb.pairings_rank_range(C, rank, world)
+    rows = end - begin
+    terms_rank = rows << (2 * n - 1 - C)
+    terms_job = 1 << (2 * n - 1)
+    stream = torch.cuda.current_stream().cuda_stream
+    out = torch.empty((rows, m), dtype=torch.int32, device="cuda")
+    host_rows = torch.empty((rows, m), dtype=torch.int32).pin_memory()
+    host_ptr = ctypes.cast(host_rows.data_ptr(), ctypes.POINTER(ctypes.c_uint32))
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
+    opts = pb.LaunchOpts(variant=pb.VARIANT_AUTO)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def step_device():
+        pb.count_pairings_ex(kind, n, C, begin, end, moduli, out.data_ptr(), stream, opts)
+
+    def finish(rows_tensor):
+        """rows -> per-rank sum -> exchange -> CRT on rank 0 (outside the timed region for `value`)."""
+        flat = (ctypes.c_uint32 * (rows * m)).from_address(rows_tensor.data_ptr())
+        total = pb.pairings_sum_rows(flat, moduli)
+        if dist is not None:
+            t = torch.tensor(total, dtype=torch.int64, device="cuda")
+            gathered = [torch.zeros_like(t) for _ in range(world)]
+            dist.all_gather(gathered, t)
+            total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
+        if rank == 0:
+            D, S = pb.pairings_reconstruct(kind, n, moduli, total)
+            assert S == L20_IDENTIFIED and D == 2 * S, ("L(20) mismatch", D, S)
+        return total
+
+    # ---- warm-up (>= 3), correctness of the warmed-up path
+    for _ in range(max(args.warmup, 3) if args.warmup >= 0 else 3):
+        step_device()
+        flush.fill_(1)
+    torch.cuda.synchronize()
+    host_rows.copy_(out)
+    finish(host_rows)
+
+    # ---- phi (exact non-zero fraction) from the kernel's own counter, untimed
+    nzt = torch.zeros(1, dtype=torch.int64, device="cuda")
+    o2 = pb.LaunchOpts(variant=pb.VARIANT_AUTO)
+    o2.nonzero_terms = nzt.data_ptr()
+    pb.count_pairings_ex(kind, n, C, begin, end, moduli, out.data_ptr(), stream, o2)
+    torch.cuda.synchronize()
+    phi = float(nzt.item()) / terms_rank
+
+    # ---- timed: K steps, CUDA events per step on the launching stream, L2 flushed between steps
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.3)
+    barrier()
+    t_begin = time.perf_counter()
+    evs = []
+    for _ in range(args.steps):
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        step_device()
+        e1.record()
+        evs.append((e0, e1))
+        flush.fill_(1)
+    barrier()
+    t_end = time.perf_counter()
+    clocks = sampler.stop(t_begin, t_end)
+    dev_ms = sum(a.elapsed_time(b) for a, b in evs)
+    if dist is not None:
+        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dev_ms = float(t.item())
+    launches = args.steps                       # one kernel launch per step and rank (grid = chunks of the rank)
+    value = terms_job * args.steps / (dev_ms * 1e-3)
+    kernel_s = dev_ms * 1e-3 / args.steps
+
+    # ---- e2e: the public host-buffer call, wall clock, copies + allocation inside
+    for _ in range(2):
+        pb.count_pairings_host(kind, n, C, begin, end, moduli, stream, opts, out=host_ptr)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        pb.count_pairings_host(kind, n, C, begin, end, moduli, stream, opts, out=host_ptr)
+        finish(host_rows)
+    barrier()
+    e2e_s = time.perf_counter() - t0
+    if dist is not None:
+        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_s = float(t.item())
+    e2e_value = terms_job * args.steps / e2e_s
+
+    line = None
+    if rank == 0:
+        ops, ys = yardstick_ops(kind, n, m, phi)
+        peak_mhz = clocks.get("sm_max_mhz") or 1965.0
+        peak = SM_COUNT * LANES_PER_SM_CLK * peak_mhz * 1e6
+        achieved = ops * (terms_rank / kernel_s)           # this rank's kernel: algorithmic thread-instr/s
+        roofline = dict(bound="alu", achieved=achieved / 1e12, peak=peak / 1e12, unit="Tinstr/s",
+                        frac=achieved / peak, traffic=None,
+                        peak_source="formula: 148 SM x 128 lanes/clk x %.0f MHz (clocks.max.sm); MEASURED_PEAKS.json has no integer figure" % peak_mhz,
+                        ops_per_term=ops, yardstick=ys,
+                        kernel_ms=kernel_s * 1e3, terms_per_launch=terms_rank)
+        # calibration kernels: measured thread-instr/s per instruction class
+        cal = {}
+        scratch = torch.zeros(4, dtype=torch.int32, device="cuda")
+        for mode, name in ((0, "iadd3"), (1, "lop3"), (2, "imad"), (3, "iadd3_imad_1to1")):
+            best = 0.0
+            for rep in range(3):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                cnt = pb.pairings_issue_probe(mode, SM_COUNT * 8, 256, 4096, scratch.data_ptr(), stream)
+                e1.record()
+                torch.cuda.synchronize()
+                best = max(best, cnt / (e0.elapsed_time(e1) * 1e-3))
+            cal[name] = best / 1e12
+        roofline["calibration_Tinstr_per_s"] = cal
+        roofline["frac_of_best_calibration"] = achieved / 1e12 / max(cal.values())
+
+        # secondary point of the metric: S(24) on the seeded 1/64 subset
+        n24 = None
+        if not args.no_n24:
+            k2, n2, C2, m2 = WL24["kind"], WL24["n"], WL24["chunk_bits"], WL24["n_moduli"]
+            mod2 = pb.pairings_default_moduli(m2)
+            starts = seeds.sample_range_starts(C2, max(1, int(WL24["runs"] * args.n24_fraction)), WL24["run_len"])
+            out2 = torch.empty((WL24["run_len"], m2), dtype=torch.int32, device="cuda")
+            pb.count_pairings_ex(k2, n2, C2, starts[0], starts[0] + WL24["run_len"], mod2, out2.data_ptr(), stream, opts)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for s0 in starts:
+                pb.count_pairings_ex(k2, n2, C2, s0, s0 + WL24["run_len"], mod2, out2.data_ptr(), stream, opts)
+            e1.record()
+            torch.cuda.synchronize()
+            t24 = e0.elapsed_time(e1) * 1e-3
+            terms24 = len(starts) * WL24["run_len"] << (2 * n2 - 1 - C2)
+            n24 = dict(workload="S(24): %d seeded runs of %d contiguous chunks of the 2^20-chunk partition, 8+1 primes" % (len(starts), WL24["run_len"]),
+                       terms=terms24, seconds=t24, value=terms24 / t24, unit="terms/s",
+                       projected_full_run_s=(1 << 47) / (terms24 / t24))
+
+        cpu = cpu_baseline(kind, n) if not args.no_cpu else None
+        line = dict(metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s", n_gpus=world,
+                    steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=dev_ms / args.steps,
+                    higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
+                    config=dict(workload="L(20): Langford n=20, 2^39 sign vectors (x_1=+1), 2^16 prefix chunks, 6 CRT primes + 1 check prime, full count per step",
+                                kind="langford", n=n, chunk_bits=C, n_moduli=m, parallelism="chunk ranges x%d" % world,
+                                l2="flushed between steps (256 MiB fill); the kernel reads no global memory",
+                                result_check="L(20) = 2,636,337,861,200 reconstructed every run (PAPER.md:380)",
+                                library=pb.pairings_build_info()),
+                    clocks=clocks,
+                    e2e=dict(value=e2e_value, unit="terms/s", h2d_bytes_per_step=4 * m + 8 * 5,
+                             d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps),
+                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24,
+                    paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")
+    if dist is not None:
+        dist.barrier()
+        dist.destroy_process_group()
+    if line is not None:
+        print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
+    ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 256 seeded S(24) runs to time")
+    ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_gpu(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -197,6 +197,13 @@ int pairings_reconstruct(int kind, int n,
 int pairings_crt_signed(const uint32_t* moduli, int n_moduli, const uint32_t* residues,
                         char* out_dec, size_t cap);
 
+/* Measurement helper (not on the path): enqueues an integer-issue calibration kernel — independent
+ * chains (ILP 8) of mode 0: IADD3, 1: LOP3, 2: IMAD, 3: IADD3:IMAD 1:1 — and reports how many
+ * thread-instructions of that class it executes, for the roofline denominator.
+ * out_dev: DEVICE, at least one uint32 (scratch). */
+int pairings_issue_probe(int mode, int blocks, int threads, int iters, uint32_t* out_dev, void* stream,
+                         uint64_t* thread_instructions);
+
 const char* pairings_strerror(int code);
 
 /* Library build string: version, CUDA arch, compiled SWAR specialisations. */

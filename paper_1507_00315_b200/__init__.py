@@ -11,5 +11,6 @@ from .api import (  # noqa: F401
     pairings_partition, pairings_rank_range, pairings_sum_rows,
     pairings_journal_append, pairings_journal_load, pairings_run,
     pairings_reconstruct, pairings_crt_signed, pairings_strerror, pairings_build_info,
+    pairings_issue_probe,
     count,
 )

@@ -62,6 +62,7 @@ def lib():
         "pairings_run": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, u32p, u64p]),
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
+        "pairings_issue_probe": (i, [i, i, i, i, vp, vp, u64p]),
         "pairings_strerror": (cp, [i]),
         "pairings_build_info": (cp, []),
     }
@@ -211,6 +212,14 @@ def pairings_crt_signed(moduli, residues) -> int:
     a = ctypes.create_string_buffer(_CAP)
     _check(lib().pairings_crt_signed(_u32(moduli), len(moduli), _u32(residues), a, _CAP), "pairings_crt_signed")
     return int(a.value)
+
+
+def pairings_issue_probe(mode: int, blocks: int, threads: int, iters: int, out_dev_ptr: int, stream: int = 0) -> int:
+    """Enqueues the calibration kernel; returns the number of thread-instructions it executes."""
+    cnt = ctypes.c_uint64(0)
+    _check(lib().pairings_issue_probe(mode, blocks, threads, iters, ctypes.c_void_p(out_dev_ptr),
+                                      ctypes.c_void_p(stream), ctypes.byref(cnt)), "pairings_issue_probe")
+    return int(cnt.value)
 
 
 def count(kind: int, n: int, chunk_bits: Optional[int] = None, n_moduli: Optional[int] = None,

@@ -69,8 +69,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
     stamp = _deps_stamp()
     srcs = sources()
-    if force:
-        for f in glob.glob(os.path.join(OBJ, "*.o")):
+    for f in glob.glob(os.path.join(OBJ, "*.o")):
+        if force or not f.endswith("." + stamp + ".o"):     # stale objects of older header states
             os.remove(f)
     with concurrent.futures.ThreadPoolExecutor(max_workers=os.cpu_count() or 4) as ex:
         objs = list(ex.map(lambda s: _compile(s, stamp, verbose), srcs))

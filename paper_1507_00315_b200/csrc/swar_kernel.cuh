@@ -43,7 +43,8 @@ namespace swar {
 constexpr int H = 4;              // unrolled inner Gray bits
 constexpr int BLK = 1 << H;       // steps per unrolled block
 constexpr int QCAP = 256;         // ring entries per warp (power of two)
-constexpr int CHECK_EVERY = 4;    // steps between drain checks; 31 + 32*CHECK_EVERY < QCAP
+constexpr int QUAD = 4;           // steps between drain checks; 31 + 32*QUAD < QCAP
+constexpr int PLANE_BYTES = QCAP * 16;   // ring = planes of 16 bytes per entry (conflict-free 128-bit accesses)
 
 #define PAIRINGS_HD __host__ __device__ constexpr
 
@@ -105,6 +106,7 @@ struct Lay {
     static constexpr int W = (term_bits() + 33 + 31) / 32;
     static_assert(W >= G && W <= 8, "accumulator must hold the multi-word product");
     static constexpr int EW = NR + 1;                   // ring entry words (packed sums + sign)
+    static constexpr int PLANES = (EW + 3) / 4;         // 16-byte planes per entry
     static constexpr uint32_t PAD = 0x40;               // value of unused slots (never reads as zero)
 };
 
@@ -233,23 +235,51 @@ __device__ __forceinline__ void acc_add_signed(uint32_t (&acc)[W], const uint32_
     }
 }
 
+__device__ __forceinline__ void sts_v4_pred(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t pred) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.shared.v4.u32 [%0], {%1, %2, %3, %4};\n\t}"
+                 :: "r"(addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void sts_v2_pred(uint32_t addr, uint32_t a, uint32_t b, uint32_t pred) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p st.shared.v2.u32 [%0], {%1, %2};\n\t}"
+                 :: "r"(addr), "r"(a), "r"(b), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void sts_v1_pred(uint32_t addr, uint32_t a, uint32_t pred) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.shared.u32 [%0], %1;\n\t}"
+                 :: "r"(addr), "r"(a), "r"(pred) : "memory");
+}
+__device__ __forceinline__ void lds_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
+    asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
+}
+
+// sign-extended byte i of w (one PRMT: selector nibble i, then three times "replicate its sign")
+template <int i>
+__device__ __forceinline__ int sbyte(uint32_t w) {
+    uint32_t r;   // (__byte_perm masks the selector's replicate-sign bits, prmt.b32 does not)
+    asm("prmt.b32 %0, %1, 0, %2;" : "=r"(r) : "r"(w), "n"(0x8880 + 0x1111 * i));
+    return (int)r;
+}
+
+// One ring entry (at shared byte address `addr` in plane 0) -> signed multi-word term -> acc.
 template <int KIND, int NN>
-__device__ __forceinline__ void drain_entry(const uint32_t* __restrict__ ring, uint32_t idx,
-                                            uint32_t (&acc)[Lay<KIND, NN>::W]) {
+__device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<KIND, NN>::W]) {
     using L = Lay<KIND, NN>;
-    constexpr int NR = L::NR, G = L::G, W = L::W;
+    constexpr int NR = L::NR, G = L::G, W = L::W, PL = L::PLANES;
+    uint32_t e[4 * PL];
+    static_for<0, PL>([&](auto pc) {
+        PAIRINGS_IC(pl, pc);
+        lds_v4(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
+    });
     uint32_t w[NR];
 #pragma unroll
-    for (int r = 0; r < NR; r++) w[r] = ring[r * QCAP + idx] ^ 0x80808080u;      // bytes -> two's complement Q
+    for (int r = 0; r < NR; r++) w[r] = e[r] ^ 0x80808080u;                       // bytes -> two's complement Q
     int gp[G];
 #pragma unroll
     for (int g = 0; g < G; g++) gp[g] = 1;
-    gp[0] = (int)ring[NR * QCAP + idx];                                           // sign of the term
+    gp[0] = (int)e[NR];                                                           // sign of the term
     static_for<0, NN>([&](auto sc) {
         PAIRINGS_IC(s, sc);
-        const int q = (int)(int8_t)(w[s / 4] >> (8 * (s % 4)));
         constexpr int g = L::group_of_slot(s);
-        gp[g] *= q;                                                               // exact: |group| < 2^31
+        gp[g] *= sbyte<s % 4>(w[s / 4]);                                          // exact: |group| < 2^31
     });
     // sign-magnitude: multi-word product of |gp[i]|
     uint32_t sx = 0;
@@ -291,28 +321,34 @@ struct Walker {
     uint32_t tail, head;      // warp-uniform ring counters (monotone)
     uint32_t sgn_even, sgn_odd;   // sign word pushed at even / odd inner steps (+1 / -1 as int)
     uint32_t ltmask;
-    uint32_t* ring;
+    uint32_t ring;            // shared-window byte address of this warp's ring (plane 0)
     int lane;
 
     __device__ __forceinline__ void push_if_nonzero(uint32_t sgnword) {
         uint32_t z = 0;
 #pragma unroll
         for (int r = 0; r < NT; r++) z |= Q[r] & ~(Q[r] - 0x01010101u);
-        const bool nonzero = (z & 0x80808080u) == 0;
-        const uint32_t bal = __ballot_sync(0xffffffffu, nonzero);
-        if (nonzero) {
-            const uint32_t idx = (tail + __popc(bal & ltmask)) & (QCAP - 1);
+        const uint32_t nonzero = ((z & 0x80808080u) == 0) ? 1u : 0u;
+        const uint32_t bal = __ballot_sync(0xffffffffu, nonzero != 0);
+        const uint32_t addr = ring + (((tail + __popc(bal & ltmask)) & (QCAP - 1)) << 4);
+        // entry words: Q[0..NR), sign; plane p holds words 4p..4p+3 (predicated vector stores, no branch)
+        uint32_t e[4 * L::PLANES];
 #pragma unroll
-            for (int r = 0; r < NR; r++) ring[r * QCAP + idx] = Q[r];
-            ring[NR * QCAP + idx] = sgnword;
-        }
+        for (int i = 0; i < 4 * L::PLANES; i++) e[i] = (i < NR) ? Q[i] : sgnword;
+        static_for<0, L::PLANES>([&](auto pc) {
+            PAIRINGS_IC(pl, pc);
+            constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
+            if constexpr (words >= 3) sts_v4_pred(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], nonzero);
+            else if constexpr (words == 2) sts_v2_pred(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], nonzero);
+            else sts_v1_pred(addr + pl * PLANE_BYTES, e[4 * pl], nonzero);
+        });
         tail += __popc(bal);
     }
 
     __device__ __forceinline__ void drain_full() {
         while (tail - head >= 32u) {
             __syncwarp();
-            drain_entry<KIND, NN>(ring, (head + (uint32_t)lane) & (QCAP - 1), acc);
+            drain_entry<KIND, NN>(ring + (((head + (uint32_t)lane) & (QCAP - 1)) << 4), acc);
             head += 32u;
             __syncwarp();
         }
@@ -321,16 +357,18 @@ struct Walker {
     __device__ __forceinline__ void drain_rest() {
         drain_full();
         __syncwarp();
-        if ((uint32_t)lane < tail - head) drain_entry<KIND, NN>(ring, (head + (uint32_t)lane) & (QCAP - 1), acc);
+        if ((uint32_t)lane < tail - head) drain_entry<KIND, NN>(ring + (((head + (uint32_t)lane) & (QCAP - 1)) << 4), acc);
         head = tail;
         __syncwarp();
     }
 
-    template <int PAR, int S>
-    __device__ __forceinline__ void inner_steps() {
-        if constexpr (S < BLK) {
+    // QUAD consecutive steps of the unrolled inner block of parity PAR, starting at step QUAD*QI:
+    // test + push the current term, then flip inner bit ctz(S+1) (nothing after the block's last step).
+    template <int PAR, int QI>
+    __device__ __forceinline__ void quad() {
+        static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
+            PAIRINGS_IC(S, sc);
             push_if_nonzero((S & 1) ? sgn_odd : sgn_even);
-            if constexpr ((S + 1) % CHECK_EVERY == 0) drain_full();
             if constexpr (S + 1 < BLK) {
                 constexpr int bi = ctz_c(S + 1);
                 constexpr int xo = 1 - 2 * ((zbits(PAR, S) >> bi) & 1);              // old x_j
@@ -341,8 +379,7 @@ struct Walker {
                     else Q[r] = Q[r] + C[bi][r] + K;
                 });
             }
-            inner_steps<PAR, S + 1>();
-        }
+        });
     }
 
     // flip of index bit b >= H (between two inner blocks)
@@ -426,22 +463,34 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     Wk wk;
     wk.lane = lane;
     wk.ltmask = (1u << lane) - 1u;
-    wk.ring = rings + (size_t)warp * (QCAP * L::EW);
+    wk.ring = (uint32_t)__cvta_generic_to_shared(rings) + (uint32_t)warp * (uint32_t)(L::PLANES * PLANE_BYTES);
     wk.tail = 0; wk.head = 0;
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
     unsigned long long nz = 0;
+    const uint32_t nquad = nblk * (BLK / QUAD);
 
     for (uint64_t q = sub * per_block + threadIdx.x; q < (sub + 1) * per_block; q += blockDim.x) {
         wk.init_prefix(chunk_base | (q << g));
         const uint32_t tail0 = wk.tail;
-        for (uint32_t tout = 0; tout < nblk; tout += 2) {
-            wk.template inner_steps<0, 0>();
-            if (tout + 1 < nblk) {
-                wk.template outer_flip<H>();                           // tout+1 is odd: always bit H
-                wk.template inner_steps<1, 0>();
-                if (tout + 2 < nblk) wk.template outer_flip_dispatch<H + 1>(H + (__ffs((int)(tout + 2)) - 1));
+        // One drain site for all steps: the unrolled quads are the cases of a (warp-uniform) switch.
+#pragma unroll 1
+        for (uint32_t qd = 0; qd < nquad; qd++) {
+            switch (qd & 7u) {
+                case 0: wk.template quad<0, 0>(); break;
+                case 1: wk.template quad<0, 1>(); break;
+                case 2: wk.template quad<0, 2>(); break;
+                case 3: wk.template quad<0, 3>();
+                        if (qd + 1 < nquad) wk.template outer_flip<H>();                 // next block index is odd: bit H
+                        break;
+                case 4: wk.template quad<1, 0>(); break;
+                case 5: wk.template quad<1, 1>(); break;
+                case 6: wk.template quad<1, 2>(); break;
+                default: wk.template quad<1, 3>();
+                        if (qd + 1 < nquad) wk.template outer_flip_dispatch<H + 1>(H + (__ffs((int)((qd + 1) >> 2)) - 1));
+                        break;
             }
+            wk.drain_full();
         }
         nz += (unsigned long long)(wk.tail - tail0);
     }
@@ -475,7 +524,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
 template <int KIND, int NN>
 int launch(const KernelParams& kp, int block_threads, unsigned grid, void* stream) {
     using L = Lay<KIND, NN>;
-    const size_t smem = (size_t)(8 * PAIRINGS_MAX_MODULI * 2 + (block_threads / 32) * QCAP * L::EW) * sizeof(uint32_t);
+    const size_t smem = (size_t)(8 * PAIRINGS_MAX_MODULI * 2) * sizeof(uint32_t) + (size_t)(block_threads / 32) * L::PLANES * PLANE_BYTES;
     cudaError_t e = cudaFuncSetAttribute(swar_kernel<KIND, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
     swar_kernel<KIND, NN><<<grid, block_threads, smem, (cudaStream_t)stream>>>(kp);
