@@ -207,9 +207,11 @@ def run_gpu(args):
     kind, n, C, m = WL["kind"], WL["n"], WL["chunk_bits"], WL["n_moduli"]
     moduli = pb.pairings_default_moduli(m)
     begin, end = pb.pairings_rank_range(C, rank, world)
+    if args.profile_chunks:                      # short launches for ncu captures; not a bench value
+        end = min(end, begin + args.profile_chunks)
     rows = end - begin
     terms_rank = rows << (2 * n - 1 - C)
-    terms_job = 1 << (2 * n - 1)
+    terms_job = (1 << (2 * n - 1)) if not args.profile_chunks else terms_rank * world
     stream = torch.cuda.current_stream().cuda_stream
     out = torch.empty((rows, m), dtype=torch.int32, device="cuda")
     host_rows = torch.empty((rows, m), dtype=torch.int32).pin_memory()
@@ -234,7 +236,7 @@ def run_gpu(args):
             gathered = [torch.zeros_like(t) for _ in range(world)]
             dist.all_gather(gathered, t)
             total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
-        if rank == 0:
+        if rank == 0 and not args.profile_chunks:
             D, S = pb.pairings_reconstruct(kind, n, moduli, total)
             assert S == L20_IDENTIFIED and D == 2 * S, ("L(20) mismatch", D, S)
         return total
@@ -357,6 +359,7 @@ def run_gpu(args):
                     clocks=clocks,
                     e2e=dict(value=e2e_value, unit="terms/s", h2d_bytes_per_step=4 * m + 8 * 5,
                              d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps),
+                    profile_only=bool(args.profile_chunks),
                     gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24,
                     paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")
     if dist is not None:
@@ -375,6 +378,8 @@ def main():
     ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
     ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 256 seeded S(24) runs to time")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--profile-chunks", type=int, default=0,
+                    help="profiling aid: only the first N chunks per step (short launches for ncu); the line is marked, not a bench value")
     args = ap.parse_args()
     if args.impl == "reference":
         run_reference(args)
