@@ -1,0 +1,56 @@
+"""N > 1 host path on CPU (gloo, world_size 2): each rank owns a contiguous chunk range
+(pairings_rank_range), sums its rows, the per-rank sums are exchanged and rank 0 reconstructs.
+The rows themselves come from the CPU oracle here (no GPU on this box); on the GPU box bench.py runs
+the same exchange around count_pairings."""
+import os
+import socket
+
+import pytest
+
+torch = pytest.importorskip("torch")
+import torch.distributed as dist
+import torch.multiprocessing as mp
+
+
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def _worker(rank, world, port, kind, n, C, q):
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    import oracle
+    import paper_1507_00315_b200 as pb
+    moduli = pb.pairings_default_moduli(pb.pairings_min_moduli(kind, n) + 1)
+    b, e = pb.pairings_rank_range(C, rank, world)
+    rows = [oracle.chunk(kind, n, C, c, moduli)[2] for c in range(b, e)]
+    mine = pb.pairings_sum_rows(rows, moduli)
+    t = torch.tensor(mine, dtype=torch.int64)
+    gathered = [torch.zeros_like(t) for _ in range(world)]
+    dist.all_gather(gathered, t)
+    total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
+    if rank == 0:
+        q.put((b, e, pb.pairings_reconstruct(kind, n, moduli, total)))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("kind,n,C,want", [(1, 8, 4, (300, 150)), (0, 9, 5, (2656, 1328)), (0, 7, 3, (0, 0))])
+def test_two_ranks_disjoint_ranges_then_crt(kind, n, C, want):
+    from paper_1507_00315_b200 import build as pbuild
+    pbuild.build()
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_worker, args=(r, 2, port, kind, n, C, q)) for r in range(2)]
+    [p.start() for p in procs]
+    b, e, got = q.get(timeout=120)
+    [p.join(timeout=120) for p in procs]
+    assert all(p.exitcode == 0 for p in procs)
+    assert (b, e) == (0, 1 << (C - 1))
+    assert got == want          # L(8)=150, S(9)=1,328, S(7): no pairing
