@@ -1,0 +1,57 @@
+"""Command line: the whole path for one (kind, n), with journal / resume.
+
+    python -m paper_1507_00315_b200 S 24 [--chunk-bits 20] [--moduli 9] [--chunks-per-call 8192]
+                                         [--journal FILE] [--max-calls K] [--json]
+
+Prints D(n) (reflections distinct) and S(n) / L(n) (reflections identified, the paper's numbers,
+PAPER.md:63) and the wall time.  Calls only the C ABI (pairings_run + pairings_reconstruct); an
+interrupted run (--max-calls, or a crash) continues from the journal when started again.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import sys
+import time
+
+from . import api
+
+
+def main(argv=None) -> int:
+    ap = argparse.ArgumentParser(prog="python -m paper_1507_00315_b200")
+    ap.add_argument("kind", choices=["S", "L", "s", "l"], help="S = Skolem (d_k = k), L = Langford (d_k = k+1)")
+    ap.add_argument("n", type=int)
+    ap.add_argument("--chunk-bits", type=int, default=None)
+    ap.add_argument("--moduli", type=int, default=None, help="CRT primes + 1 check prime (default: north_star bound + 1)")
+    ap.add_argument("--chunks-per-call", type=int, default=1 << 13)
+    ap.add_argument("--journal", default=None)
+    ap.add_argument("--max-calls", type=int, default=0)
+    ap.add_argument("--json", action="store_true")
+    a = ap.parse_args(argv)
+
+    kind = api.SKOLEM if a.kind.upper() == "S" else api.LANGFORD
+    n = a.n
+    m = a.moduli if a.moduli is not None else api.pairings_bound_moduli(kind, n) + 1
+    moduli = api.pairings_default_moduli(m)
+    C = a.chunk_bits if a.chunk_bits is not None else max(0, min(2 * n - 1 - 17, 20))
+    t0 = time.perf_counter()
+    total, done = api.pairings_run(kind, n, C, moduli, a.chunks_per_call, a.journal, a.max_calls)
+    dt = time.perf_counter() - t0
+    res = dict(kind=a.kind.upper(), n=n, chunk_bits=C, moduli=moduli, chunks_done=done, chunks=1 << C,
+               seconds=dt, total_residues=total)
+    if done == 1 << C:
+        D, S = api.pairings_reconstruct(kind, n, moduli, total)
+        res.update(distinct=D, identified=S, terms=1 << (2 * n - 1), terms_per_s=(1 << (2 * n - 1)) / dt)
+    if a.json:
+        print(json.dumps(res))
+    elif done == 1 << C:
+        print("%s(%d): reflections identified %d, distinct %d  (%.2f s in this call, %d chunks)" %
+              (res["kind"], n, res["identified"], res["distinct"], dt, done))
+    else:
+        print("%s(%d): %d of %d chunks done (%.2f s in this call); run again to continue" %
+              (res["kind"], n, done, 1 << C, dt))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -32,6 +32,7 @@
 
 #include "internal.h"
 #include "device_common.cuh"
+#include "swar_list.h"
 
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -40,11 +41,12 @@
 namespace pairings {
 namespace swar {
 
-constexpr int H = 4;              // unrolled inner Gray bits
+constexpr int H = PAIRINGS_SWAR_H;              // unrolled inner Gray bits
 constexpr int BLK = 1 << H;       // steps per unrolled block
 constexpr int QCAP = 256;         // ring entries per warp (power of two)
 constexpr int QUAD = 4;           // steps between drain checks; 31 + 32*QUAD < QCAP
 constexpr int PLANE_BYTES = QCAP * 16;   // ring = planes of 16 bytes per entry (conflict-free 128-bit accesses)
+constexpr int RING_ALIGN = PLANE_BYTES;  // plane 0 of every ring is PLANE_BYTES-aligned: slot address = ring | offset
 
 #define PAIRINGS_HD __host__ __device__ constexpr
 
@@ -120,8 +122,10 @@ __device__ __forceinline__ uint32_t spread4(uint32_t x) { return (x * 0x00204081
 // index bit b at distance d_s; it always exists for b <= n-3), as a 32-bit integer per register:
 //     out[r] = sum_{s in r} unit(s) * x * 256^{s%4}      (signed bytes added as integers).
 // INNER: only neighbours outside the inner bits (b + d_s >= H) are included.
-// !INNER: the RIGHT neighbours (index bit b - d_s >= 0) are added too; at the moment bit b flips in
-//         Gray order bit b-1 is 1 and all lower bits are 0, so they are compile-time constants.
+// !INNER: the RIGHT neighbours (index bit b - d_s >= 0) are added too; at the moment outer bit b flips
+//         the inner bits are all 0 (every block starts and ends there, see Walker::block_end), outer
+//         bit b-1 is 1 (Gray order over the outer bits) and the outer bits below it are 0, so they
+//         are compile-time constants.
 template <int KIND, int NN, int b, bool INNER>
 struct LeftVec {
     using L = Lay<KIND, NN>;
@@ -143,7 +147,7 @@ struct LeftVec {
             const int s = 4 * r + o;
             if (s >= NN) continue;
             const int d = L::d_of_slot(s), u = L::unit(s);
-            if (!INNER && d <= b) v += (uint32_t)(d == 1 ? -u : u) << (8 * o);   // right neighbour, known
+            if (!INNER && d <= b) v += (uint32_t)((d == 1 && b > H) ? -u : u) << (8 * o);   // right neighbour, known
             if (included(s)) v += (uint32_t)u << (8 * o);                          // x = +1 part of the left neighbour
         }
         return v;
@@ -171,14 +175,13 @@ struct LeftVec {
 // ------------------------------------------------------------------------------------------------
 // compile-time constants of the unrolled inner blocks
 // ------------------------------------------------------------------------------------------------
-// inner state (bit set <-> x = -1) at inner step S of a block with parity PAR
-PAIRINGS_HD int zbits(int par, int s) { return gray_c(s) ^ (par << (H - 1)); }
+// inner state (bit set <-> x = -1) at inner step S of a block: every block starts at 0
+PAIRINGS_HD int zbits(int s) { return gray_c(s); }
 
-// K: contribution of the inner neighbours to dQ when inner bit bi = ctz(S+1) flips at step S -> S+1
+// K: contribution of the inner neighbours to dQ when inner bit bi flips in inner state zb
 template <int KIND, int NN>
-PAIRINGS_HD uint32_t kconst(int par, int S, int r) {
+PAIRINGS_HD uint32_t kconst(int zb, int bi, int r) {
     using L = Lay<KIND, NN>;
-    const int zb = zbits(par, S), bi = ctz_c(S + 1);
     const int xo = 1 - 2 * ((zb >> bi) & 1);
     uint32_t K = 0;
     for (int o = 0; o < 4; o++) {
@@ -318,11 +321,11 @@ struct Walker {
     uint32_t C[H][NR];
     uint32_t E, O;            // de-interleaved sign word: E bit i = index bit 2i, O bit i = index bit 2i+1
     uint32_t acc[W];
-    uint32_t tail, head;      // warp-uniform ring counters (monotone)
+    uint32_t tail16, head16;  // warp-uniform ring counters (monotone), in units of 1/16 entry (= byte offsets)
     uint32_t sgn_even, sgn_odd;   // sign word pushed at even / odd inner steps (+1 / -1 as int)
     uint32_t ltmask;
-    uint32_t ring;            // shared-window byte address of this warp's ring (plane 0)
-    int lane;
+    uint32_t ring;            // shared-window byte address of this warp's ring (plane 0), RING_ALIGN-aligned
+    uint32_t lane16;          // lane * 16
 
     __device__ __forceinline__ void push_if_nonzero(uint32_t sgnword) {
         uint32_t z = 0;
@@ -330,7 +333,8 @@ struct Walker {
         for (int r = 0; r < NT; r++) z |= Q[r] & ~(Q[r] - 0x01010101u);
         const uint32_t nonzero = ((z & 0x80808080u) == 0) ? 1u : 0u;
         const uint32_t bal = __ballot_sync(0xffffffffu, nonzero != 0);
-        const uint32_t addr = ring + (((tail + __popc(bal & ltmask)) & (QCAP - 1)) << 4);
+        // slot = (tail + rank among the warp's non-zero lanes) mod QCAP; ring is aligned, so "|" adds the offset
+        const uint32_t addr = ((tail16 + 16u * (uint32_t)__popc(bal & ltmask)) & (uint32_t)(PLANE_BYTES - 16)) | ring;
         // entry words: Q[0..NR), sign; plane p holds words 4p..4p+3 (predicated vector stores, no branch)
         uint32_t e[4 * L::PLANES];
 #pragma unroll
@@ -342,14 +346,18 @@ struct Walker {
             else if constexpr (words == 2) sts_v2_pred(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], nonzero);
             else sts_v1_pred(addr + pl * PLANE_BYTES, e[4 * pl], nonzero);
         });
-        tail += __popc(bal);
+        tail16 += 16u * (uint32_t)__popc(bal);
+    }
+
+    __device__ __forceinline__ uint32_t slot_of_lane() const {
+        return ((head16 + lane16) & (uint32_t)(PLANE_BYTES - 16)) | ring;
     }
 
     __device__ __forceinline__ void drain_full() {
-        while (tail - head >= 32u) {
+        while (tail16 - head16 >= 32u * 16u) {
             __syncwarp();
-            drain_entry<KIND, NN>(ring + (((head + (uint32_t)lane) & (QCAP - 1)) << 4), acc);
-            head += 32u;
+            drain_entry<KIND, NN>(slot_of_lane(), acc);
+            head16 += 32u * 16u;
             __syncwarp();
         }
     }
@@ -357,29 +365,41 @@ struct Walker {
     __device__ __forceinline__ void drain_rest() {
         drain_full();
         __syncwarp();
-        if ((uint32_t)lane < tail - head) drain_entry<KIND, NN>(ring + (((head + (uint32_t)lane) & (QCAP - 1)) << 4), acc);
-        head = tail;
+        if (lane16 < tail16 - head16) drain_entry<KIND, NN>(slot_of_lane(), acc);
+        head16 = tail16;
         __syncwarp();
     }
 
-    // QUAD consecutive steps of the unrolled inner block of parity PAR, starting at step QUAD*QI:
-    // test + push the current term, then flip inner bit ctz(S+1) (nothing after the block's last step).
-    template <int PAR, int QI>
+    // QUAD consecutive steps of the unrolled inner block, starting at step QUAD*QI: test + push the
+    // current term, then flip inner bit ctz(S+1) (the block's last step is followed by block_end).
+    template <int QI>
     __device__ __forceinline__ void quad() {
         static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
             PAIRINGS_IC(S, sc);
             push_if_nonzero((S & 1) ? sgn_odd : sgn_even);
-            if constexpr (S + 1 < BLK) {
-                constexpr int bi = ctz_c(S + 1);
-                constexpr int xo = 1 - 2 * ((zbits(PAR, S) >> bi) & 1);              // old x_j
-                static_for<0, NR>([&](auto rc) {
-                    PAIRINGS_IC(r, rc);
-                    constexpr uint32_t K = kconst<KIND, NN>(PAR, S, r);
-                    if constexpr (xo > 0) Q[r] = Q[r] - C[bi][r] + K;                // dQ = -x_j * C + K
-                    else Q[r] = Q[r] + C[bi][r] + K;
-                });
-            }
+            if constexpr (S + 1 < BLK) inner_flip<zbits(S), ctz_c(S + 1)>();
         });
+    }
+
+    // flip of inner bit bi in inner state ZB: dQ = -x_j * C[bi] + K  (row a3; K = inner neighbours, folded)
+    template <int ZB, int bi>
+    __device__ __forceinline__ void inner_flip() {
+        constexpr int xo = 1 - 2 * ((ZB >> bi) & 1);                                 // old x_j
+        static_for<0, NR>([&](auto rc) {
+            PAIRINGS_IC(r, rc);
+            constexpr uint32_t K = kconst<KIND, NN>(ZB, bi, r);
+            if constexpr (xo > 0) Q[r] = Q[r] - C[bi][r] + K;
+            else Q[r] = Q[r] + C[bi][r] + K;
+        });
+    }
+
+    // Between two blocks: the inner walk ended in state 1 << (H-1); flip that bit back so that every
+    // block runs the same compile-time sequence from inner state 0, then flip outer bit `bit`.  The
+    // two flips keep the sign of the term, so the signs pushed at even / odd steps swap.
+    __device__ __forceinline__ void block_end(int bit) {
+        inner_flip<(1 << (H - 1)), H - 1>();
+        outer_flip_dispatch<H>(bit);
+        const uint32_t t = sgn_even; sgn_even = sgn_odd; sgn_odd = t;
     }
 
     // flip of index bit b >= H (between two inner blocks)
@@ -447,9 +467,13 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     using Wk = Walker<KIND, NN>;
     constexpr int N = L::N, B = N - 1, W = L::W;
     extern __shared__ uint32_t smem[];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = blockDim.x >> 5;
-    unsigned long long* red = reinterpret_cast<unsigned long long*>(smem);              // 8 * 16 uint64
-    uint32_t* rings = smem + 8 * PAIRINGS_MAX_MODULI * 2;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    // dynamic shared memory: [alignment slack][rings: warps x PLANES x PLANE_BYTES][reduction scratch]
+    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t rings = (smem_base + (uint32_t)(RING_ALIGN - 1)) & ~(uint32_t)(RING_ALIGN - 1);
+    const uint32_t ring_bytes = (blockDim.x >> 5) * (uint32_t)(L::PLANES * PLANE_BYTES);
+    unsigned long long* red = reinterpret_cast<unsigned long long*>(
+        reinterpret_cast<unsigned char*>(smem) + (rings - smem_base) + ring_bytes);              // 8 * 16 uint64
 
     const int C = kp.chunk_bits, g = kp.gray_bits;
     const uint64_t chunk_local = (uint64_t)blockIdx.x >> kp.log2_bpc;
@@ -461,41 +485,30 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     const uint32_t nblk = 1u << (g - H);
 
     Wk wk;
-    wk.lane = lane;
+    wk.lane16 = (uint32_t)lane * 16u;
     wk.ltmask = (1u << lane) - 1u;
-    wk.ring = (uint32_t)__cvta_generic_to_shared(rings) + (uint32_t)warp * (uint32_t)(L::PLANES * PLANE_BYTES);
-    wk.tail = 0; wk.head = 0;
+    wk.ring = rings + (uint32_t)warp * (uint32_t)(L::PLANES * PLANE_BYTES);
+    wk.tail16 = 0; wk.head16 = 0;
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
     unsigned long long nz = 0;
-    const uint32_t nquad = nblk * (BLK / QUAD);
 
     for (uint64_t q = sub * per_block + threadIdx.x; q < (sub + 1) * per_block; q += blockDim.x) {
         wk.init_prefix(chunk_base | (q << g));
-        const uint32_t tail0 = wk.tail;
-        // One drain site for all steps: the unrolled quads are the cases of a (warp-uniform) switch.
+        const uint32_t tail0 = wk.tail16;
+        // One inner block = BLK unrolled steps from inner state 0, a drain check every QUAD steps.
 #pragma unroll 1
-        for (uint32_t qd = 0; qd < nquad; qd++) {
-            switch (qd & 7u) {
-                case 0: wk.template quad<0, 0>(); break;
-                case 1: wk.template quad<0, 1>(); break;
-                case 2: wk.template quad<0, 2>(); break;
-                case 3: wk.template quad<0, 3>();
-                        if (qd + 1 < nquad) wk.template outer_flip<H>();                 // next block index is odd: bit H
-                        break;
-                case 4: wk.template quad<1, 0>(); break;
-                case 5: wk.template quad<1, 1>(); break;
-                case 6: wk.template quad<1, 2>(); break;
-                default: wk.template quad<1, 3>();
-                        if (qd + 1 < nquad) wk.template outer_flip_dispatch<H + 1>(H + (__ffs((int)((qd + 1) >> 2)) - 1));
-                        break;
-            }
-            wk.drain_full();
+        for (uint32_t u = 0; u < nblk; u++) {
+            static_for<0, BLK / QUAD>([&](auto qc) {
+                PAIRINGS_IC(QI, qc);
+                wk.template quad<QI>();
+                wk.drain_full();
+            });
+            if (u + 1 < nblk) wk.block_end(H + (__ffs((int)(u + 1)) - 1));      // Gray order over the outer bits
         }
-        nz += (unsigned long long)(wk.tail - tail0);
+        nz += (unsigned long long)((wk.tail16 - tail0) >> 4);
     }
     wk.drain_rest();
-    (void)nwarps;
 
     // ---- once per thread: accumulator (W-word two's complement) -> residues, times 2^{#even}
     uint32_t vals[PAIRINGS_MAX_MODULI];
@@ -524,7 +537,8 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
 template <int KIND, int NN>
 int launch(const KernelParams& kp, int block_threads, unsigned grid, void* stream) {
     using L = Lay<KIND, NN>;
-    const size_t smem = (size_t)(8 * PAIRINGS_MAX_MODULI * 2) * sizeof(uint32_t) + (size_t)(block_threads / 32) * L::PLANES * PLANE_BYTES;
+    const size_t smem = (size_t)RING_ALIGN + (size_t)(block_threads / 32) * L::PLANES * PLANE_BYTES
+                      + (size_t)(8 * PAIRINGS_MAX_MODULI * 2) * sizeof(uint32_t);
     cudaError_t e = cudaFuncSetAttribute(swar_kernel<KIND, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
     swar_kernel<KIND, NN><<<grid, block_threads, smem, (cudaStream_t)stream>>>(kp);

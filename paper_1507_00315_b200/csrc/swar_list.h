@@ -1,6 +1,8 @@
 // (kind, n) pairs the SWAR kernel is compiled for: X(kind, n).  One object file per entry
 // (build.py compiles swar_inst.cu once per entry with -DPAIRINGS_SWAR_KIND / -DPAIRINGS_SWAR_N).
 // Values of n where pairings exist, from the smallest the kernel supports (n-2 >= 4).
+// unrolled inner Gray bits of the SWAR kernel (smallest gray_bits it accepts)
+#define PAIRINGS_SWAR_H 5
 #ifndef PAIRINGS_SWAR_LIST
 #define PAIRINGS_SWAR_LIST(X) \
     X(0, 8) X(0, 12) X(0, 13) X(0, 16) X(0, 20) X(0, 21) X(0, 24) \

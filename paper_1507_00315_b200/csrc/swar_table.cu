@@ -15,7 +15,7 @@ swar_launch_fn swar_lookup(int kind, int n) {
     return nullptr;
 }
 
-int swar_min_gray_bits() { return 4; }
+int swar_min_gray_bits() { return PAIRINGS_SWAR_H; }
 
 const char* swar_list() {
 #define PAIRINGS_STR(k, nn) #k ":" #nn " "

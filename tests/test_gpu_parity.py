@@ -47,7 +47,7 @@ def oracle_rows(kind, n, C, chunks, moduli, threads=8):
 
 def variant_available(variant, kind, n, C):
     if variant == pb.VARIANT_SWAR:
-        return pb.pairings_has_swar(kind, n) and (2 * n - 1 - C) >= 9   # >= 32 prefixes of >= 2^4 steps per chunk
+        return pb.pairings_has_swar(kind, n) and (2 * n - 1 - C) >= 10   # >= 32 prefixes of >= 2^5 steps per chunk
     return True
 
 
@@ -94,7 +94,7 @@ def test_geometry_never_changes_the_rows(variant):
         pytest.skip("variant not compiled")
     moduli = pb.pairings_default_moduli(4)
     ref = gpu_rows(kind, n, C, 0, 1 << C, moduli, pb.LaunchOpts(variant=variant))
-    gs = [4, 7, 10] if variant == pb.VARIANT_SWAR else [0, 1, 5, 12, 17]
+    gs = [5, 7, 10] if variant == pb.VARIANT_SWAR else [0, 1, 5, 12, 17]
     for g in gs:
         for threads, bpc in ((32, 1), (128, 2), (256, 1), (64, 8)):
             if bpc * threads > (1 << (2 * n - 1 - C - g)) and (bpc > 1 or variant == pb.VARIANT_SWAR):
