@@ -85,27 +85,75 @@ struct Lay {
     PAIRINGS_HD static int bound(int s) { return d_of_slot(s) % 2 == 0 ? cnt(s) / 2 : cnt(s); }   // |Q| <= bound
     static constexpr int NR = (NN + 3) / 4;            // packed registers
     static constexpr int NT = (n_even() + 3) / 4;      // registers that need the zero test
-    // greedy grouping of slots into exact signed 32-bit products
-    PAIRINGS_HD static int group_of_slot(int s) {
-        int g = 0; uint64_t prod = 1;
-        for (int t = 0; t <= s; t++) {
-            if (prod * (uint64_t)bound(t) >= (1ULL << 31)) { g++; prod = 1; }
-            prod *= (uint64_t)bound(t);
+    // ---- product plan (row a5).  The n factors are multiplied as "pair factors": byte i of register
+    // 2p times byte i of register 2p+1 in ONE dp4a (the second operand masked to that byte), bytes
+    // (0,1) and (2,3) of an unpaired last register likewise; a slot without a partner is a single
+    // sign-extracted byte.  Pair factors are then packed (best fit, decreasing) into G groups whose
+    // exact signed products stay below 2^31.
+    static constexpr int NF_MAX = 4 * ((NR + 1) / 2) + 4;
+    struct Plan {
+        int nf;                    // number of factors
+        int kind[NF_MAX];          // 1: registers (r, r+1) byte i;  2: register r bytes (i, i+1);  3: register r byte i alone
+        int r[NF_MAX], i[NF_MAX];
+        uint64_t bound[NF_MAX];    // |factor| <= bound
+        int group[NF_MAX];
+        int G;                     // number of groups
+        int bits;                  // sum over groups of bitlen(bound of the group product)
+        bool unbias[NR];           // register needs its own  ^ 0x80808080  (used as a dp4a first operand or for single bytes)
+    };
+    PAIRINGS_HD static uint64_t slot_bound(int s) { return s < NN ? (uint64_t)bound(s) : 0; }
+    PAIRINGS_HD static Plan make_plan(bool last_as_singles) {
+        Plan P{};
+        int nf = 0;
+        for (int r = 0; r < NR; r++) P.unbias[r] = false;
+        for (int p = 0; 2 * p + 1 < NR; p++) {
+            const int r = 2 * p;
+            for (int i = 0; i < 4; i++) {
+                const uint64_t b1 = slot_bound(4 * r + i), b2 = slot_bound(4 * (r + 1) + i);
+                if (b1 && b2) { P.kind[nf] = 1; P.r[nf] = r; P.i[nf] = i; P.bound[nf] = b1 * b2; nf++; P.unbias[r] = true; }
+                else if (b1) { P.kind[nf] = 3; P.r[nf] = r; P.i[nf] = i; P.bound[nf] = b1; nf++; P.unbias[r] = true; }
+            }
         }
-        return g;
-    }
-    PAIRINGS_HD static int n_groups() { return group_of_slot(NN - 1) + 1; }
-    PAIRINGS_HD static int term_bits() {                // upper bound on bitlen(|prod_k Q_k|)
-        int bits = 0, g = 0; uint64_t prod = 1;
-        for (int t = 0; t < NN; t++) {
-            if (group_of_slot(t) != g) { bits += bitlen_c(prod); prod = 1; g = group_of_slot(t); }
-            prod *= (uint64_t)bound(t);
+        if (NR % 2 == 1) {
+            const int r = NR - 1;
+            for (int i = 0; i < 4; i += (last_as_singles ? 1 : 2)) {
+                const uint64_t b1 = slot_bound(4 * r + i), b2 = last_as_singles ? 0 : slot_bound(4 * r + i + 1);
+                if (b1 && b2) { P.kind[nf] = 2; P.r[nf] = r; P.i[nf] = i; P.bound[nf] = b1 * b2; nf++; P.unbias[r] = true; }
+                else if (b1) { P.kind[nf] = 3; P.r[nf] = r; P.i[nf] = i; P.bound[nf] = b1; nf++; P.unbias[r] = true; }
+            }
         }
-        return bits + bitlen_c(prod);
+        P.nf = nf;
+        // best-fit decreasing into the fewest groups with product < 2^31
+        int order[NF_MAX] = {};
+        for (int f = 0; f < nf; f++) order[f] = f;
+        for (int a = 0; a < nf; a++)
+            for (int c = a + 1; c < nf; c++)
+                if (P.bound[order[c]] > P.bound[order[a]]) { const int t = order[a]; order[a] = order[c]; order[c] = t; }
+        for (int G = 1; G <= 8; G++) {
+            uint64_t prod[8] = {1, 1, 1, 1, 1, 1, 1, 1};
+            bool ok = true;
+            for (int a = 0; a < nf && ok; a++) {
+                const int f = order[a];
+                int best = -1;
+                for (int g = 0; g < G; g++)
+                    if (prod[g] * P.bound[f] < (1ULL << 31) && (best < 0 || prod[g] > prod[best])) best = g;
+                if (best < 0) ok = false; else { prod[best] *= P.bound[f]; P.group[f] = best; }
+            }
+            if (ok) {
+                P.G = G; P.bits = 0;
+                for (int g = 0; g < G; g++) P.bits += bitlen_c(prod[g]);
+                return P;
+            }
+        }
+        P.G = 0;                                       // does not happen for n <= 32 (static_assert below)
+        return P;
     }
-    static constexpr int G = n_groups();
-    // accumulator words: |sum| < 2^term_bits * 2^32 drained terms per thread (host enforces), + sign
-    static constexpr int W = (term_bits() + 33 + 31) / 32;
+    // finer factors for an unpaired last register only where that saves a group (n = 20: G = 3 instead of 4)
+    static constexpr Plan plan = make_plan(true).G < make_plan(false).G ? make_plan(true) : make_plan(false);
+    static constexpr int G = plan.G;
+    // accumulator words: |sum| < 2^bits * 2^32 drained terms per thread (host enforces), + sign
+    static constexpr int W = (plan.bits + 33 + 31) / 32;
+    static_assert(G >= 1, "no grouping found");
     static_assert(W >= G && W <= 8, "accumulator must hold the multi-word product");
     static constexpr int EW = NR + 1;                   // ring entry words (packed sums + sign)
     static constexpr int PLANES = (EW + 3) / 4;         // 16-byte planes per entry
@@ -272,17 +320,35 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
         PAIRINGS_IC(pl, pc);
         lds_v4(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
     });
+    uint32_t c80 = 0x80808080u;
+    asm("" : "+r"(c80));                                                          // keep it in a register: one LOP3 per masked operand
     uint32_t w[NR];
-#pragma unroll
-    for (int r = 0; r < NR; r++) w[r] = e[r] ^ 0x80808080u;                       // bytes -> two's complement Q
+    static_for<0, NR>([&](auto rc) {                                              // bytes -> two's complement Q
+        PAIRINGS_IC(r, rc);
+        constexpr bool ub = L::plan.unbias[r];
+        w[r] = ub ? (e[r] ^ 0x80808080u) : 0u;
+    });
     int gp[G];
 #pragma unroll
     for (int g = 0; g < G; g++) gp[g] = 1;
     gp[0] = (int)e[NR];                                                           // sign of the term
-    static_for<0, NN>([&](auto sc) {
-        PAIRINGS_IC(s, sc);
-        constexpr int g = L::group_of_slot(s);
-        gp[g] *= sbyte<s % 4>(w[s / 4]);                                          // exact: |group| < 2^31
+    static_for<0, L::NF_MAX>([&](auto fc) {
+        PAIRINGS_IC(f, fc);
+        if constexpr (f < L::plan.nf) {
+            constexpr int kind = L::plan.kind[f], r = L::plan.r[f], i = L::plan.i[f], g = L::plan.group[f];
+            int v;
+            if constexpr (kind == 1) {          // Q[4r+i] * Q[4(r+1)+i]: second operand = ((e ^ 0x80..) & byte i)
+                uint32_t b;
+                asm("lop3.b32 %0, %1, %2, %3, 0x28;" : "=r"(b) : "r"(e[r + 1]), "r"(c80), "n"(0xFFu << (8 * i)));
+                v = __dp4a((int)w[r], (int)b, 0);
+            } else if constexpr (kind == 2) {   // Q[4r+i] * Q[4r+i+1]: second operand = byte i+1 moved to byte i
+                const uint32_t b = __byte_perm(w[r], 0, i == 0 ? 0x4441 : 0x4344);
+                v = __dp4a((int)w[r], (int)b, 0);
+            } else {
+                v = sbyte<i>(w[r]);
+            }
+            gp[g] *= v;                                                           // exact: |group| < 2^31
+        }
     });
     // sign-magnitude: multi-word product of |gp[i]|
     uint32_t sx = 0;
