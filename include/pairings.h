@@ -177,6 +177,27 @@ int pairings_run(int kind, int n, int chunk_bits,
                  void* stream, const pairings_launch_opts* opts,
                  uint32_t* total_out, uint64_t* chunks_done_out);
 
+/* §8(f) NEXT #1 — symmetry 3 (Lemma 2.4; the paper fixes a second variable with it,
+ * PAPER.md:253).  With x^ = (x_1, -x_2, x_3, -x_4, ...):  term(x^) = (-1)^{n + sum_k d_k} term(x).
+ * Returns 1 if the exponent is even (term(x^) = term(x): Skolem n = 0,1 mod 4, Langford n = 0,3 mod 4 —
+ * exactly the n for which pairings exist), so the x_2 = +1 half of the sum is H/2;
+ * 0 if it is odd (term(x^) = -term(x): the two halves cancel and H = 0); negative code on invalid (kind, n). */
+int pairings_lemma24(int kind, int n);
+
+/* pairings_run with flags.  PAIRINGS_RUN_LEMMA24: use symmetry 3 — x_2 is the most significant chunk
+ * bit, so only chunks [0, 2^{chunk_bits-1}) are evaluated (none at all when pairings_lemma24 is 0) and
+ * the sum is doubled at the end; needs chunk_bits >= 1, otherwise the flag is ignored.
+ *   *chunks_needed_out (may be NULL) = number of chunks this mode evaluates in total.
+ *   When *chunks_done_out == *chunks_needed_out, total_out holds H mod p_i (symmetry factor applied);
+ *   before that it is the raw partial sum.  A journal that already holds chunks of the x_2 = -1 half
+ *   (written by a run without the flag) is refused with PAIRINGS_EJOURNAL. */
+enum { PAIRINGS_RUN_LEMMA24 = 1 };
+int pairings_run_ex(int kind, int n, int chunk_bits,
+                    const uint32_t* moduli, int n_moduli,
+                    uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                    void* stream, const pairings_launch_opts* opts, unsigned flags,
+                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out);
+
 /* §8(a) row a7 — CRT reconstruction ("the actual value is obtained using the chinese
  * remainder theorem") and the exact division of Lemma 2.1.
  *   moduli[0..n_moduli-2] are the CRT primes, moduli[n_moduli-1] is the redundant check prime

@@ -1,7 +1,7 @@
 """Command line: the whole path for one (kind, n), with journal / resume.
 
     python -m paper_1507_00315_b200 S 24 [--chunk-bits 20] [--moduli 9] [--chunks-per-call 8192]
-                                         [--journal FILE] [--max-calls K] [--json]
+                                         [--journal FILE] [--max-calls K] [--lemma24] [--json]
 
 Prints D(n) (reflections distinct) and S(n) / L(n) (reflections identified, the paper's numbers,
 PAPER.md:63) and the wall time.  Calls only the C ABI (pairings_run + pairings_reconstruct); an
@@ -23,7 +23,9 @@ def main(argv=None) -> int:
     ap.add_argument("n", type=int)
     ap.add_argument("--chunk-bits", type=int, default=None)
     ap.add_argument("--moduli", type=int, default=None, help="CRT primes + 1 check prime (default: north_star bound + 1)")
-    ap.add_argument("--chunks-per-call", type=int, default=1 << 13)
+    ap.add_argument("--chunks-per-call", type=int, default=None)
+    ap.add_argument("--lemma24", action="store_true",
+                    help="symmetry 3 (Lemma 2.4, PAPER.md:215-249): evaluate only the x_2 = +1 half and double it")
     ap.add_argument("--journal", default=None)
     ap.add_argument("--max-calls", type=int, default=0)
     ap.add_argument("--json", action="store_true")
@@ -33,23 +35,26 @@ def main(argv=None) -> int:
     n = a.n
     m = a.moduli if a.moduli is not None else api.pairings_bound_moduli(kind, n) + 1
     moduli = api.pairings_default_moduli(m)
-    C = a.chunk_bits if a.chunk_bits is not None else max(0, min(2 * n - 1 - 17, 20))
+    C = a.chunk_bits if a.chunk_bits is not None else api.default_chunk_bits(n)
+    per_call = a.chunks_per_call if a.chunks_per_call is not None else api.default_chunks_per_call(n, C)
     t0 = time.perf_counter()
-    total, done = api.pairings_run(kind, n, C, moduli, a.chunks_per_call, a.journal, a.max_calls)
+    total, done, needed = api.pairings_run_ex(kind, n, C, moduli, per_call, a.journal, a.max_calls, 0, None,
+                                              api.RUN_LEMMA24 if a.lemma24 else 0)
     dt = time.perf_counter() - t0
-    res = dict(kind=a.kind.upper(), n=n, chunk_bits=C, moduli=moduli, chunks_done=done, chunks=1 << C,
-               seconds=dt, total_residues=total)
-    if done == 1 << C:
+    res = dict(kind=a.kind.upper(), n=n, chunk_bits=C, moduli=moduli, chunks_done=done, chunks_needed=needed,
+               chunks=1 << C, lemma24=bool(a.lemma24), seconds=dt, total_residues=total)
+    if done == needed:
         D, S = api.pairings_reconstruct(kind, n, moduli, total)
-        res.update(distinct=D, identified=S, terms=1 << (2 * n - 1), terms_per_s=(1 << (2 * n - 1)) / dt)
+        evaluated = needed << (2 * n - 1 - C)
+        res.update(distinct=D, identified=S, terms_evaluated=evaluated, terms_per_s=evaluated / dt if dt > 0 else None)
     if a.json:
         print(json.dumps(res))
-    elif done == 1 << C:
+    elif done == needed:
         print("%s(%d): reflections identified %d, distinct %d  (%.2f s in this call, %d chunks)" %
               (res["kind"], n, res["identified"], res["distinct"], dt, done))
     else:
         print("%s(%d): %d of %d chunks done (%.2f s in this call); run again to continue" %
-              (res["kind"], n, done, 1 << C, dt))
+              (res["kind"], n, done, needed, dt))
     return 0
 
 

@@ -60,6 +60,8 @@ def lib():
         "pairings_journal_append": (i, [cp, i, i, i, u32p, i, u64, u64, u32p]),
         "pairings_journal_load": (ctypes.c_int64, [cp, i, i, i, u32p, i, u64p, ctypes.c_int64, u32p]),
         "pairings_run": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, u32p, u64p]),
+        "pairings_run_ex": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, ctypes.c_uint, u32p, u64p, u64p]),
+        "pairings_lemma24": (i, [i, i]),
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
         "pairings_issue_probe": (i, [i, i, i, i, vp, vp, u64p]),
@@ -200,6 +202,27 @@ def pairings_run(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=None
     return [int(t[j]) for j in range(k)], int(done.value)
 
 
+RUN_LEMMA24 = 1
+
+
+def pairings_lemma24(kind: int, n: int) -> int:
+    """1: term(x^) = term(x) (pairings exist); 0: term(x^) = -term(x) (H = 0).  Lemma 2.4."""
+    return _check(lib().pairings_lemma24(kind, n), "pairings_lemma24")
+
+
+def pairings_run_ex(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=None, max_calls=0, stream: int = 0,
+                    opts: Optional[LaunchOpts] = None, flags: int = 0):
+    """Whole-job host driver with flags.  Returns (total residues, chunks done, chunks needed)."""
+    k = len(moduli)
+    t = _u32([0] * k)
+    done, needed = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    jp = os.fsencode(journal_path) if journal_path is not None else None
+    _check(lib().pairings_run_ex(kind, n, chunk_bits, _u32(moduli), k, chunks_per_call, jp, max_calls,
+                                 ctypes.c_void_p(stream), _opts(opts), flags, t, ctypes.byref(done),
+                                 ctypes.byref(needed)), "pairings_run_ex")
+    return [int(t[j]) for j in range(k)], int(done.value), int(needed.value)
+
+
 def pairings_reconstruct(kind, n, moduli, total_residues):
     """Returns (D, S) = (reflections distinct, reflections identified) as Python ints."""
     a, b = ctypes.create_string_buffer(_CAP), ctypes.create_string_buffer(_CAP)
@@ -222,14 +245,28 @@ def pairings_issue_probe(mode: int, blocks: int, threads: int, iters: int, out_d
     return int(cnt.value)
 
 
+def default_chunk_bits(n: int) -> int:
+    """2^23 sign vectors per chunk (one block of 256 threads x 2^15 terms), at most 2^20 chunks."""
+    return max(0, min(2 * n - 1 - 23, 20))
+
+
+def default_chunks_per_call(n: int, chunk_bits: int) -> int:
+    """About 2^38 sign vectors per kernel call (a fraction of a second): few launches, journal lines, D2H copies."""
+    return 1 << max(0, min(chunk_bits, 38 - (2 * n - 1 - chunk_bits)))
+
+
 def count(kind: int, n: int, chunk_bits: Optional[int] = None, n_moduli: Optional[int] = None,
-          chunks_per_call: int = 1 << 12, journal_path=None, opts: Optional[LaunchOpts] = None):
+          chunks_per_call: Optional[int] = None, journal_path=None, opts: Optional[LaunchOpts] = None,
+          lemma24: bool = False):
     """Convenience: the whole path for (kind, n) -> (D, S).  Calls only the C ABI."""
     if n_moduli is None:
         n_moduli = pairings_bound_moduli(kind, n) + 1
     moduli = pairings_default_moduli(n_moduli)
     if chunk_bits is None:
-        chunk_bits = max(0, min(2 * n - 1 - 17, 20))
-    total, done = pairings_run(kind, n, chunk_bits, moduli, chunks_per_call, journal_path, 0, 0, opts)
-    assert done == 1 << chunk_bits
+        chunk_bits = default_chunk_bits(n)
+    if chunks_per_call is None:
+        chunks_per_call = default_chunks_per_call(n, chunk_bits)
+    total, done, needed = pairings_run_ex(kind, n, chunk_bits, moduli, chunks_per_call, journal_path, 0, 0, opts,
+                                          RUN_LEMMA24 if lemma24 else 0)
+    assert done == needed
     return pairings_reconstruct(kind, n, moduli, total)

@@ -305,15 +305,30 @@ int count_pairings_host(int kind, int n, int chunk_bits, uint64_t chunk_begin, u
     return PAIRINGS_OK;
 }
 
-int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
-                 uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
-                 void* stream, const pairings_launch_opts* opts,
-                 uint32_t* total_out, uint64_t* chunks_done_out) {
+int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                    uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                    void* stream, const pairings_launch_opts* opts, unsigned flags,
+                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out) {
     int rc = validate(kind, n, chunk_bits, 0, 0, moduli, n_moduli, total_out); if (rc) return rc;
     if (!total_out || !chunks_done_out) return PAIRINGS_ENULL;
     if (chunks_per_call == 0) return PAIRINGS_EINVAL_CHUNK;
+    if (flags & ~(unsigned)PAIRINGS_RUN_LEMMA24) return PAIRINGS_EINVAL_OPTS;
     for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
     *chunks_done_out = 0;
+
+    // Lemma 2.4: negating the even positions maps the x_2 = +1 half of every
+    // sum onto the x_2 = -1 half, term for term (up to the sign pairings_lemma24 reports).  The most
+    // significant chunk bit is x_2, so the x_2 = +1 half is the chunk range [0, 2^{C-1}).
+    uint64_t needed = 1ULL << chunk_bits;
+    uint32_t multiplier = 1;
+    if ((flags & PAIRINGS_RUN_LEMMA24) && chunk_bits >= 1) {
+        const int sym = pairings_lemma24(kind, n);
+        if (sym < 0) return sym;
+        if (sym == 1) { needed >>= 1; multiplier = 2; }
+        else { needed = 0; multiplier = 0; }           // the two halves cancel: H = 0, nothing to evaluate
+    }
+    if (chunks_needed_out) *chunks_needed_out = needed;
+    if (needed == 0) return PAIRINGS_OK;
 
     // a1: what is already journalled
     std::vector<uint64_t> done;
@@ -325,8 +340,12 @@ int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_
         nd = pairings_journal_load(journal_path, kind, n, chunk_bits, moduli, n_moduli, done.data(), nd, total_out);
         if (nd < 0) return (int)nd;
         done.resize((size_t)(2 * nd));
-        for (int64_t j = 0; j < nd; j++) *chunks_done_out += done[(size_t)(2 * j + 1)] - done[(size_t)(2 * j)];
+        for (int64_t j = 0; j < nd; j++) {
+            if (done[(size_t)(2 * j + 1)] > needed) return PAIRINGS_EJOURNAL;   // journal of a run without the symmetry
+            *chunks_done_out += done[(size_t)(2 * j + 1)] - done[(size_t)(2 * j)];
+        }
     }
+    if (needed < (1ULL << chunk_bits)) { done.push_back(needed); done.push_back(1ULL << chunk_bits); }   // not to be evaluated
     // a1: the remaining ranges
     int64_t need = pairings_partition(chunk_bits, chunks_per_call, done.data(), (int)(done.size() / 2), nullptr, 0);
     if (need < 0) return (int)need;
@@ -352,7 +371,18 @@ int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_
         *chunks_done_out += e - b;
         calls++;
     }
+    if (*chunks_done_out == needed && multiplier == 2) {       // complete: H = 2 * (x_2 = +1 half)
+        rc = pairings_sum_rows(total_out, 1, moduli, n_moduli, total_out); if (rc) return rc;
+    }
     return PAIRINGS_OK;
+}
+
+int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                 uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                 void* stream, const pairings_launch_opts* opts,
+                 uint32_t* total_out, uint64_t* chunks_done_out) {
+    return pairings_run_ex(kind, n, chunk_bits, moduli, n_moduli, chunks_per_call, journal_path, max_calls,
+                           stream, opts, 0u, total_out, chunks_done_out, nullptr);
 }
 
 const char* pairings_build_info(void) {

@@ -246,6 +246,15 @@ int pairings_bound_moduli(int kind, int n) {
     return PAIRINGS_ERANGE;
 }
 
+int pairings_lemma24(int kind, int n) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    // x^ = (x_1, -x_2, x_3, -x_4, ...): P_d(x^) = (-1)^d P_d(x) and prod_i x^_i = (-1)^n prod_i x_i, so
+    // term(x^) = (-1)^{n + sum_k d_k} term(x)   (Lemma 2.4, written out for both kinds).
+    long e = n;
+    for (int k = 1; k <= n; k++) e += dist(kind, k);
+    return (e % 2 == 0) ? 1 : 0;
+}
+
 int64_t pairings_partition(int chunk_bits, uint64_t max_chunks, const uint64_t* done, int n_done,
                            uint64_t* out_ranges, int64_t cap_ranges) {
     if (chunk_bits < 0 || chunk_bits > 63 || max_chunks == 0 || n_done < 0) return PAIRINGS_EINVAL_CHUNK;

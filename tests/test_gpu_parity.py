@@ -32,16 +32,26 @@ def gpu_rows(kind, n, C, begin, end, moduli, opts=None, count_nonzero=False):
     return (rows, int(nz.item())) if count_nonzero else rows
 
 
-def oracle_rows(kind, n, C, chunks, moduli, threads=8):
-    out = [None] * len(chunks)
+def oracle_rows(kind, n, C, chunks, moduli, threads=8, pieces=1):
+    """oracle.chunk for every chunk, on host threads; `pieces` > 1 cuts each chunk's index range into
+    equal sub-ranges (oracle.range_sum) whose exact sums are added here, so that a few large chunks
+    still use every core."""
+    w = 1 << (2 * n - 1 - C)
+    jobs = [(i, c * w + j * (w // pieces), c * w + (j + 1) * (w // pieces)) for i, c in enumerate(chunks) for j in range(pieces)]
+    parts = [None] * len(jobs)
 
     def work(tid):
-        for i in range(tid, len(chunks), threads):
-            out[i] = oracle.chunk(kind, n, C, chunks[i], moduli)
+        for k in range(tid, len(jobs), threads):
+            parts[k] = oracle.range_sum(kind, n, jobs[k][1], jobs[k][2], moduli)
 
     ts = [threading.Thread(target=work, args=(t,)) for t in range(threads)]
     [t.start() for t in ts]
     [t.join() for t in ts]
+    out = []
+    for i in range(len(chunks)):
+        mine = [parts[k] for k in range(len(jobs)) if jobs[k][0] == i]
+        out.append((sum(p[0] for p in mine), sum(p[1] for p in mine),
+                    [sum(p[2][j] for p in mine) % moduli[j] for j in range(len(moduli))]))
     return out
 
 
@@ -192,3 +202,63 @@ def test_host_buffer_call_and_run_driver_with_journal(tmp_path):
     total2, done2 = pb.pairings_run(kind, n, C, moduli, 256, path)                # nothing left to do
     assert (total2, done2) == (total, 256)
     assert pb.count(S, 13) == (3040560, 1520280)                                 # config 2, both conventions
+
+
+@pytest.mark.parametrize("kind,n", [(S, 12), (S, 13), (L, 11), (L, 12), (S, 10), (L, 9), (S, 16), (L, 16)])
+def test_lemma24_half_run_gives_the_same_count(kind, n, paper_counts, tmp_path):
+    # §8(f) NEXT #1: symmetry 3 (Lemma 2.4) in the host driver: half the chunks, doubled
+    C = 8
+    moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)
+    path = str(tmp_path / "j.txt")
+    total, done, needed = pb.pairings_run_ex(kind, n, C, moduli, 48, path, 0, 0, None, pb.RUN_LEMMA24)
+    if (kind, n) in paper_counts:
+        assert done == needed == 128
+        full, fdone = pb.pairings_run(kind, n, C, moduli, 256) if n <= 13 else (total, 256)
+        assert total == full and fdone == 256
+        D, Sid = pb.pairings_reconstruct(kind, n, moduli, total)
+        assert Sid == paper_counts[(kind, n)] and D == 2 * Sid
+        # resumed from the complete journal: nothing to do, same answer; a full run refuses nothing either
+        assert pb.pairings_run_ex(kind, n, C, moduli, 48, path, 0, 0, None, pb.RUN_LEMMA24) == (total, 128, 128)
+    else:
+        assert (done, needed) == (0, 0) and pb.pairings_reconstruct(kind, n, moduli, total) == (0, 0)
+        full, fdone = pb.pairings_run(kind, n, C, moduli, 256)
+        assert pb.pairings_reconstruct(kind, n, moduli, full) == (0, 0)
+
+
+def test_lemma24_refuses_a_journal_of_the_other_half(tmp_path):
+    kind, n, C = L, 12, 6
+    moduli = pb.pairings_default_moduli(4)
+    path = str(tmp_path / "j.txt")
+    pb.pairings_run(kind, n, C, moduli, 64, path)                       # full run: journal covers [0, 64)
+    with pytest.raises(pb.PairingsError) as e:
+        pb.pairings_run_ex(kind, n, C, moduli, 64, path, 0, 0, None, pb.RUN_LEMMA24)
+    assert e.value.code == -11
+
+
+# ---- BASELINE configs 4 and 5 at full size, in the launch configuration bench.py times: rows of seeded
+# chunks against the oracle one by one (each oracle chunk is 2^23 .. 2^27 plain evaluations).
+@pytest.mark.parametrize("kind,n,C,m,count", [(L, 20, 16, 7, 16), (S, 21, 18, 7, 16), (S, 24, 20, 9, 4)])
+def test_full_size_sampled_chunks_match_oracle(kind, n, C, m, count):
+    moduli = pb.pairings_default_moduli(m)
+    chunks = seeds.sample_chunks(C, count, salt=100 + n)
+    want = oracle_rows(kind, n, C, chunks, moduli, threads=16, pieces=16 if n == 24 else 1)
+    # the bench launches whole ranges: take each sampled chunk out of a 64-chunk launch around it
+    for c, w in zip(chunks, want):
+        b = min(c & ~63, (1 << C) - 64)
+        rows = gpu_rows(kind, n, C, b, b + 64, moduli)
+        assert rows[c - b] == w[2], (kind, n, c)
+        assert pb.pairings_crt_signed(moduli, rows[c - b]) == w[0]
+
+
+@pytest.mark.parametrize("kind,n,C", [(L, 20, 16), (S, 20, 16), (S, 21, 18)])
+def test_full_totals_match_the_paper(kind, n, C, paper_counts):
+    # PAPER.md:353-354 (Table 7: S(20), S(21)), :380 (Table 8: L(20)); one launch over every chunk, as in bench.py
+    moduli = pb.pairings_default_moduli(7)
+    out = torch.empty((1 << C, 7), dtype=torch.int32, device="cuda")
+    pb.count_pairings(kind, n, C, 0, 1 << C, moduli, out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    flat = (ctypes.c_uint32 * ((1 << C) * 7)).from_buffer_copy(out.cpu().numpy().tobytes())
+    D, Sid = pb.pairings_reconstruct(kind, n, moduli, pb.pairings_sum_rows(flat, moduli))
+    assert Sid == paper_counts[(kind, n)] and D == 2 * Sid
+    # and with symmetry 3: half the work
+    assert pb.count(kind, n, lemma24=True) == (D, Sid)

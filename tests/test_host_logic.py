@@ -240,3 +240,24 @@ def test_compute_without_gpu_fails_loudly():
     assert ei.value.code == -6
     with pytest.raises(pb.PairingsError):
         pb.pairings_run(1, 12, 6, pb.pairings_default_moduli(4), 16)
+
+
+def test_lemma24_applies_exactly_where_pairings_exist():
+    # PAPER.md:41,49 (existence) and PAPER.md:215-249 (Lemma 2.4; the Langford case by the same argument)
+    for n in range(2, 33):
+        assert pb.pairings_lemma24(pb.SKOLEM, n) == (1 if n % 4 in (0, 1) else 0)
+        assert pb.pairings_lemma24(pb.LANGFORD, n) == (1 if n % 4 in (0, 3) else 0)
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_lemma24(pb.SKOLEM, 1)
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_lemma24(2, 8)
+
+
+def test_run_ex_without_pairings_needs_no_gpu():
+    # term(x^) = -term(x): the two x_2 halves cancel, H = 0, nothing is launched (so this runs on CPU)
+    moduli = pb.pairings_default_moduli(4)
+    total, done, needed = pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, pb.RUN_LEMMA24)
+    assert (total, done, needed) == ([0, 0, 0, 0], 0, 0)
+    assert pb.pairings_reconstruct(pb.SKOLEM, 10, moduli, total) == (0, 0)
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, 2)      # unknown flag

@@ -259,3 +259,15 @@ def test_chunk_index_contract():
             pre = [1] + [(-1 if (c >> (C - 1 - i)) & 1 else 1) for i in range(C)]
             want += oracle.term(kind, n, pre + list(low))
         assert oracle.chunk(kind, n, C, c)[0] == want
+
+
+@pytest.mark.parametrize("kind,n", [(k, n) for k in (S, L) for n in range(2, 10)])
+def test_lemma24_x2_half_is_half_the_sum_or_cancels(kind, n):
+    # Lemma 2.4 as the host driver uses it: chunk bit C-1 is x_2, so with C = 1 chunk 0
+    # is the x_2 = +1 half.  Where pairings exist both halves are equal; elsewhere they cancel.
+    t0, t1 = oracle.chunk(kind, n, 1, 0)[0], oracle.chunk(kind, n, 1, 1)[0]
+    exists = (n % 4 in (0, 1)) if kind == S else (n % 4 in (0, 3))
+    if exists:
+        assert t0 == t1 and 2 * t0 == oracle.brute_count(kind, n) << (2 * n - 1)
+    else:
+        assert t0 == -t1 and oracle.brute_count(kind, n) == 0
