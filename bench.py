@@ -286,6 +286,9 @@ def run_gpu(args):
     # ---- e2e: the public host-buffer call, wall clock, copies + allocation inside
     for _ in range(2):
         pb.count_pairings_host(kind, n, C, begin, end, moduli, stream, opts, out=host_ptr)
+    sampler2 = ClockSampler(local)
+    sampler2.start()
+    time.sleep(0.3)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
@@ -293,6 +296,7 @@ def run_gpu(args):
         finish(host_rows)
     barrier()
     e2e_s = time.perf_counter() - t0
+    clocks_e2e = sampler2.stop(t0, t0 + e2e_s)
     if dist is not None:
         t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
@@ -358,7 +362,8 @@ def run_gpu(args):
                                 library=pb.pairings_build_info()),
                     clocks=clocks,
                     e2e=dict(value=e2e_value, unit="terms/s", h2d_bytes_per_step=4 * m + 8 * 5,
-                             d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps),
+                             d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps,
+                             clocks=clocks_e2e),
                     profile_only=bool(args.profile_chunks),
                     gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24,
                     paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")

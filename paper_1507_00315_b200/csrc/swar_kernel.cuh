@@ -286,6 +286,47 @@ __device__ __forceinline__ void acc_add_signed(uint32_t (&acc)[W], const uint32_
     }
 }
 
+// acc += x  (W-word two's complement add with carry propagation)
+template <int W>
+__device__ __forceinline__ void acc_add(uint32_t (&acc)[W], const uint32_t (&x)[W]) {
+    static_assert(W >= 2 && W <= 8, "accumulator width");
+    if constexpr (W == 2) {
+        asm volatile("add.cc.u32 %0, %0, %2;\n\taddc.u32 %1, %1, %3;"
+                     : "+r"(acc[0]), "+r"(acc[1])
+                     : "r"(x[0]), "r"(x[1]));
+    }
+    else if constexpr (W == 3) {
+        asm volatile("add.cc.u32 %0, %0, %3;\n\taddc.cc.u32 %1, %1, %4;\n\taddc.u32 %2, %2, %5;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2])
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]));
+    }
+    else if constexpr (W == 4) {
+        asm volatile("add.cc.u32 %0, %0, %4;\n\taddc.cc.u32 %1, %1, %5;\n\taddc.cc.u32 %2, %2, %6;\n\taddc.u32 %3, %3, %7;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3])
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]));
+    }
+    else if constexpr (W == 5) {
+        asm volatile("add.cc.u32 %0, %0, %5;\n\taddc.cc.u32 %1, %1, %6;\n\taddc.cc.u32 %2, %2, %7;\n\taddc.cc.u32 %3, %3, %8;\n\taddc.u32 %4, %4, %9;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4])
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]));
+    }
+    else if constexpr (W == 6) {
+        asm volatile("add.cc.u32 %0, %0, %6;\n\taddc.cc.u32 %1, %1, %7;\n\taddc.cc.u32 %2, %2, %8;\n\taddc.cc.u32 %3, %3, %9;\n\taddc.cc.u32 %4, %4, %10;\n\taddc.u32 %5, %5, %11;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "+r"(acc[5])
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]));
+    }
+    else if constexpr (W == 7) {
+        asm volatile("add.cc.u32 %0, %0, %7;\n\taddc.cc.u32 %1, %1, %8;\n\taddc.cc.u32 %2, %2, %9;\n\taddc.cc.u32 %3, %3, %10;\n\taddc.cc.u32 %4, %4, %11;\n\taddc.cc.u32 %5, %5, %12;\n\taddc.u32 %6, %6, %13;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "+r"(acc[5]), "+r"(acc[6])
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]));
+    }
+    else if constexpr (W == 8) {
+        asm volatile("add.cc.u32 %0, %0, %8;\n\taddc.cc.u32 %1, %1, %9;\n\taddc.cc.u32 %2, %2, %10;\n\taddc.cc.u32 %3, %3, %11;\n\taddc.cc.u32 %4, %4, %12;\n\taddc.cc.u32 %5, %5, %13;\n\taddc.cc.u32 %6, %6, %14;\n\taddc.u32 %7, %7, %15;"
+                     : "+r"(acc[0]), "+r"(acc[1]), "+r"(acc[2]), "+r"(acc[3]), "+r"(acc[4]), "+r"(acc[5]), "+r"(acc[6]), "+r"(acc[7])
+                     : "r"(x[0]), "r"(x[1]), "r"(x[2]), "r"(x[3]), "r"(x[4]), "r"(x[5]), "r"(x[6]), "r"(x[7]));
+    }
+}
+
 __device__ __forceinline__ void sts_v4_pred(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t pred) {
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.shared.v4.u32 [%0], {%1, %2, %3, %4};\n\t}"
                  :: "r"(addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(pred) : "memory");
@@ -350,29 +391,70 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
             gp[g] *= v;                                                           // exact: |group| < 2^31
         }
     });
-    // sign-magnitude: multi-word product of |gp[i]|
-    uint32_t sx = 0;
+    if constexpr (G <= 3) {
+        // signed multi-word product T = gp[0] * gp[1] * ... (two's complement, top word signed).  A k-word T
+        // times a signed 32-bit m: the k-1 low (unsigned) words are multiplied by m read as unsigned, i.e.
+        // by m + 2^32 [m < 0], and that excess — the low words shifted up one word — is subtracted again.
+        uint32_t T[W];
 #pragma unroll
-    for (int g = 0; g < G; g++) sx ^= (uint32_t)gp[g];
-    const uint32_t mask = (uint32_t)((int)sx >> 31);                              // all ones iff the term is negative
-    uint32_t T[W];
+        for (int i = 0; i < W; i++) T[i] = 0;
+        T[0] = (uint32_t)gp[0];
+        static_for<1, G>([&](auto gc) {
+            PAIRINGS_IC(k, gc);                                   // T has k words before this multiplication
+            const int m = gp[k];
+            uint32_t lowT[k > 1 ? k - 1 : 1];
+            uint32_t carry = 0;
+            static_for<0, k - 1>([&](auto ic) {
+                PAIRINGS_IC(i, ic);
+                lowT[i] = T[i];
+                const uint64_t p = (uint64_t)T[i] * (uint32_t)m + carry;
+                T[i] = (uint32_t)p; carry = (uint32_t)(p >> 32);
+            });
+            int64_t top;                                          // signed top word x signed m + carry: one IMAD.WIDE
+            asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(top) : "r"((int)T[k - 1]), "r"(m), "l"((int64_t)(uint64_t)carry));
+            T[k - 1] = (uint32_t)(uint64_t)top; T[k] = (uint32_t)((uint64_t)top >> 32);
+            if constexpr (k == 2) {
+                asm("{\n\t.reg .pred p;\n\tsetp.lt.s32 p, %3, 0;\n\t@p sub.cc.u32 %0, %0, %2;\n\t@p subc.u32 %1, %1, 0;\n\t}"
+                    : "+r"(T[1]), "+r"(T[2]) : "r"(lowT[0]), "r"(m));
+            } else if constexpr (k == 3) {
+                asm("{\n\t.reg .pred p;\n\tsetp.lt.s32 p, %5, 0;\n\t@p sub.cc.u32 %0, %0, %3;\n\t@p subc.cc.u32 %1, %1, %4;\n\t@p subc.u32 %2, %2, 0;\n\t}"
+                    : "+r"(T[1]), "+r"(T[2]), "+r"(T[3]) : "r"(lowT[0]), "r"(lowT[1]), "r"(m));
+            } else if constexpr (k == 4) {
+                asm("{\n\t.reg .pred p;\n\tsetp.lt.s32 p, %7, 0;\n\t@p sub.cc.u32 %0, %0, %4;\n\t@p subc.cc.u32 %1, %1, %5;\n\t@p subc.cc.u32 %2, %2, %6;\n\t@p subc.u32 %3, %3, 0;\n\t}"
+                    : "+r"(T[1]), "+r"(T[2]), "+r"(T[3]), "+r"(T[4]) : "r"(lowT[0]), "r"(lowT[1]), "r"(lowT[2]), "r"(m));
+            } else {
+                static_assert(k == 1, "more than 5 groups: extend the correction chain");
+            }
+        });
+        const uint32_t sext = (uint32_t)((int)T[G - 1] >> 31);    // sign words above the G-word product
 #pragma unroll
-    for (int i = 0; i < W; i++) T[i] = 0;
-    T[0] = (uint32_t)abs(gp[0]);
+        for (int i = G; i < W; i++) T[i] = sext;
+        acc_add<W>(acc, T);
+    } else {
+        // sign-magnitude: multi-word product of |gp[i]|
+        uint32_t sx = 0;
 #pragma unroll
-    for (int g = 1; g < G; g++) {
-        const uint32_t m = (uint32_t)abs(gp[g]);
-        uint32_t carry = 0;
+        for (int g = 0; g < G; g++) sx ^= (uint32_t)gp[g];
+        const uint32_t mask = (uint32_t)((int)sx >> 31);                              // all ones iff the term is negative
+        uint32_t T[W];
 #pragma unroll
-        for (int i = 0; i < g; i++) {
-            const uint64_t p = (uint64_t)T[i] * m + carry;
-            T[i] = (uint32_t)p; carry = (uint32_t)(p >> 32);
+        for (int i = 0; i < W; i++) T[i] = 0;
+        T[0] = (uint32_t)abs(gp[0]);
+#pragma unroll
+        for (int g = 1; g < G; g++) {
+            const uint32_t m = (uint32_t)abs(gp[g]);
+            uint32_t carry = 0;
+#pragma unroll
+            for (int i = 0; i < g; i++) {
+                const uint64_t p = (uint64_t)T[i] * m + carry;
+                T[i] = (uint32_t)p; carry = (uint32_t)(p >> 32);
+            }
+            T[g] = carry;
         }
-        T[g] = carry;
-    }
 #pragma unroll
-    for (int i = 0; i < W; i++) T[i] ^= mask;
-    acc_add_signed<W>(acc, T, mask);
+        for (int i = 0; i < W; i++) T[i] ^= mask;
+        acc_add_signed<W>(acc, T, mask);
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
