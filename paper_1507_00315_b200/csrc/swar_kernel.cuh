@@ -8,25 +8,28 @@
 //    Q_k = P_k for odd d_k.  The factor 2^{#even} is restored once per thread at the end.
 //    Even-d slots come first, so the zero test (row a4) looks at NT = ceil(#even/4) registers:
 //    a byte is 0x80 iff  bit7(v) & ~bit7(v - 0x01010101).
-//  * the low H = 4 index bits are walked by two fully unrolled 16-step Gray blocks (block parity =
-//    state of inner bit 3).  For every inner position the packed vector C[b] of its neighbours that
-//    lie OUTSIDE the inner bits is kept in registers; neighbours inside the inner bits are known at
+//  * the low H = 5 index bits are walked by ONE fully unrolled 32-step Gray block that always starts
+//    in inner state 0.  For every inner position the packed vector C[b] of its neighbours that lie
+//    OUTSIDE the inner bits is kept in registers; neighbours inside the inner bits are known at
 //    compile time and folded into an immediate.  One Gray step (row a3) is therefore
 //         Q[r] = Q[r] -/+ C[b][r] + K[r]          — one 3-input add per register, n/4 per step,
 //    instead of n boundary-guarded updates.  (Deltas are added as whole 32-bit integers: bytes stay
 //    in [65,191] after every step, so no carry ever crosses a slot.)
-//  * index bits H..g-1 ("outer" flips, once per 16 steps) rebuild the neighbour vector of the
-//    flipped position from two de-interleaved copies (E: even index bits, O: odd) of the sign word
-//    with a multiply-spread (4 bits -> 4 bytes), and patch one byte of each C[b].
+//  * between two blocks the inner state (only bit H-1 set) is flipped back to 0 together with the
+//    outer flip (Gray order over index bits H..g-1), so every block runs the same compile-time
+//    sequence; each sign vector is still visited exactly once.  The outer flip rebuilds the neighbour
+//    vector of the flipped position from two de-interleaved copies (E: even index bits, O: odd) of
+//    the sign word with a multiply-spread (4 bits -> 4 bytes), and patches one byte of each C[b].
 //    Because g <= n-2, every left neighbour of a walked position exists: no boundary guards at all.
 //  * non-zero terms are compacted (row a4's divergence problem): ballot + popc prefix push the packed
 //    registers + sign into a per-warp shared-memory ring; whenever 32 entries are queued all lanes
 //    multiply one entry each (any lane may process any term of its warp: the sum is commutative and
 //    a warp never spans two chunks).
-//  * row a5: the product is formed as G exact signed group products (< 2^31 each), multiplied to a
-//    multi-word magnitude and added, with sign, into a W-word two's-complement accumulator.  The
-//    reduction modulo the primes happens ONCE per thread (32-bit Montgomery Horner), not per term —
-//    the residues written are identical, the per-term cost no longer depends on the number of primes.
+//  * row a5: the product is formed from dp4a "pair factors" (two sums per LOP3 + IDP.4A), G exact
+//    signed group products (< 2^31 each), a signed multi-word product, added into a W-word
+//    two's-complement accumulator.  The reduction modulo the primes happens ONCE per thread (32-bit
+//    Montgomery Horner), not per term — the residues written are identical, the per-term cost no
+//    longer depends on the number of primes.
 //  * row a6: shared with the generic kernel (block_reduce_write).
 #pragma once
 
