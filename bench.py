@@ -303,6 +303,17 @@ def run_gpu(args):
         e2e_s = float(t.item())
     e2e_value = terms_job * args.steps / e2e_s
 
+    # ---- whole count with symmetry 3 (Lemma 2.4, §8(f) NEXT #1): half the chunks, doubled; wall clock, rank 0
+    lemma24 = None
+    if rank == 0 and world == 1 and not args.profile_chunks:
+        t0 = time.perf_counter()
+        tot, done, needed = pb.pairings_run_ex(kind, n, C, moduli, 1 << C, None, 0, stream, opts, pb.RUN_LEMMA24)
+        dt = time.perf_counter() - t0
+        D, S = pb.pairings_reconstruct(kind, n, moduli, tot)
+        assert S == L20_IDENTIFIED and done == needed == 1 << (C - 1)
+        lemma24 = dict(seconds=dt, chunks_evaluated=needed, terms_evaluated=needed << (2 * n - 1 - C),
+                       note="pairings_run_ex(PAIRINGS_RUN_LEMMA24): x_2 = +1 half of the chunks, doubled; same count")
+
     line = None
     if rank == 0:
         ops, ys = yardstick_ops(kind, n, m, phi)
@@ -365,7 +376,7 @@ def run_gpu(args):
                              d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps,
                              clocks=clocks_e2e),
                     profile_only=bool(args.profile_chunks),
-                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24,
+                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24, lemma24=lemma24,
                     paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")
     if dist is not None:
         dist.barrier()

@@ -644,7 +644,11 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
     unsigned long long nz = 0;
 
-    for (uint64_t q = sub * per_block + threadIdx.x; q < (sub + 1) * per_block; q += blockDim.x) {
+    // per_block is a multiple of blockDim (host): a block-uniform trip count keeps the warps provably converged
+    const uint32_t rounds = (uint32_t)(per_block / blockDim.x);
+#pragma unroll 1
+    for (uint32_t rd = 0; rd < rounds; rd++) {
+        const uint64_t q = sub * per_block + (uint64_t)rd * blockDim.x + threadIdx.x;
         wk.init_prefix(chunk_base | (q << g));
         const uint32_t tail0 = wk.tail16;
         // One inner block = BLK unrolled steps from inner state 0, a drain check every QUAD steps.
