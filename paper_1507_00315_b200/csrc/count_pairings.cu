@@ -232,7 +232,7 @@ static int launch_range(int kind, int n, int chunk_bits, uint64_t chunk_begin, u
 
     KernelParams kp; std::memset(&kp, 0, sizeof kp);
     kp.kind = kind; kp.n = n; kp.chunk_bits = chunk_bits; kp.gray_bits = geo.g; kp.log2_bpc = geo.log2_bpc;
-    kp.n_moduli = n_moduli;
+    kp.n_moduli = n_moduli; kp.c80 = 0x80808080u;
     kp.nonzero = opts ? (unsigned long long*)opts->nonzero_terms : nullptr;
     for (int i = 0; i < n_moduli; i++) kp.primes[i] = make_prime(moduli[i]);
 

@@ -35,6 +35,8 @@ struct KernelParams {
     int gray_bits;        // g
     int log2_bpc;         // log2(blocks per chunk)
     int n_moduli;
+    uint32_t c80;         // 0x80808080, passed as data so that it stays in a register (SWAR drain: one LOP3 per masked operand)
+    uint32_t pad0;
     uint64_t chunk_begin;
     uint64_t n_chunks;
     uint32_t* out;        // DEVICE rows

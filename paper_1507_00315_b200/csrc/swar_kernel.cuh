@@ -356,7 +356,7 @@ __device__ __forceinline__ int sbyte(uint32_t w) {
 
 // One ring entry (at shared byte address `addr` in plane 0) -> signed multi-word term -> acc.
 template <int KIND, int NN>
-__device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<KIND, NN>::W]) {
+__device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<KIND, NN>::W], uint32_t c80) {
     using L = Lay<KIND, NN>;
     constexpr int NR = L::NR, G = L::G, W = L::W, PL = L::PLANES;
     uint32_t e[4 * PL];
@@ -364,8 +364,6 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
         PAIRINGS_IC(pl, pc);
         lds_v4(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
     });
-    uint32_t c80 = 0x80808080u;
-    asm("" : "+r"(c80));                                                          // keep it in a register: one LOP3 per masked operand
     uint32_t w[NR];
     static_for<0, NR>([&](auto rc) {                                              // bytes -> two's complement Q
         PAIRINGS_IC(r, rc);
@@ -477,6 +475,7 @@ struct Walker {
     uint32_t ltmask;
     uint32_t ring;            // shared-window byte address of this warp's ring (plane 0), RING_ALIGN-aligned
     uint32_t lane16;          // lane * 16
+    uint32_t c80;             // 0x80808080 (KernelParams::c80)
 
     __device__ __forceinline__ void push_if_nonzero(uint32_t sgnword) {
         uint32_t z = 0;
@@ -507,7 +506,7 @@ struct Walker {
     __device__ __forceinline__ void drain_full() {
         while (tail16 - head16 >= 32u * 16u) {
             __syncwarp();
-            drain_entry<KIND, NN>(slot_of_lane(), acc);
+            drain_entry<KIND, NN>(slot_of_lane(), acc, c80);
             head16 += 32u * 16u;
             __syncwarp();
         }
@@ -516,7 +515,7 @@ struct Walker {
     __device__ __forceinline__ void drain_rest() {
         drain_full();
         __syncwarp();
-        if (lane16 < tail16 - head16) drain_entry<KIND, NN>(slot_of_lane(), acc);
+        if (lane16 < tail16 - head16) drain_entry<KIND, NN>(slot_of_lane(), acc, c80);
         head16 = tail16;
         __syncwarp();
     }
@@ -612,7 +611,10 @@ struct Walker {
 };
 
 template <int KIND, int NN>
-__global__ void __launch_bounds__(256)
+#ifndef PAIRINGS_SWAR_MINB
+#define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM (the ring limits it to 3 anyway): at most 85 registers
+#endif
+__global__ void __launch_bounds__(256, PAIRINGS_SWAR_MINB)
 swar_kernel(const __grid_constant__ KernelParams kp) {
     using L = Lay<KIND, NN>;
     using Wk = Walker<KIND, NN>;
@@ -637,6 +639,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
 
     Wk wk;
     wk.lane16 = (uint32_t)lane * 16u;
+    wk.c80 = kp.c80;
     wk.ltmask = (1u << lane) - 1u;
     wk.ring = rings + (uint32_t)warp * (uint32_t)(L::PLANES * PLANE_BYTES);
     wk.tail16 = 0; wk.head16 = 0;
