@@ -37,6 +37,7 @@ KIND_NAME = {0: "S", 1: "L"}
 # workload (BASELINE.json configs[3]): Langford n = 20, 2^16 chunks, 6 primes + 1 check prime
 WL = dict(kind=1, n=20, chunk_bits=16, n_moduli=7)
 L20_IDENTIFIED = 2636337861200          # L(20), PAPER.md:380 (Table 8)
+WORKLOAD = "L(20): Langford n=20, 2^39 sign vectors (x_1=+1), 2^16 prefix chunks, 6 CRT primes + 1 check prime, full count per step"
 # secondary point of the metric (configs[4]): Skolem n = 24, 2^20 chunks, 8 primes + 1 check prime,
 # a fixed seeded 1/64 subset of chunks (256 runs of 64 contiguous chunks)
 WL24 = dict(kind=0, n=24, chunk_bits=20, n_moduli=9, runs=256, run_len=64)
@@ -130,7 +131,8 @@ def run_reference(args):
     line = dict(impl="reference", metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s",
                 n_gpus=args.gpus, steps=steps, warmup=warm, ms_per_step=1e3 * t_total / steps,
                 higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
-                config=dict(workload="L(20): Langford n=20, bounded oracle sample per step", sample=sample),
+                config=dict(workload=WORKLOAD, kind="langford", n=n, chunk_bits=WL["chunk_bits"], n_moduli=WL["n_moduli"],
+                            sample="each step is a bounded sample of the workload: " + sample),
                 cpu_baseline=dict(value=value, unit="terms/s", cores=threads, kind="oracle", sample=sample),
                 e2e=dict(value=value, unit="terms/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
@@ -366,7 +368,7 @@ def run_gpu(args):
         line = dict(metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s", n_gpus=world,
                     steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=dev_ms / args.steps,
                     higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
-                    config=dict(workload="L(20): Langford n=20, 2^39 sign vectors (x_1=+1), 2^16 prefix chunks, 6 CRT primes + 1 check prime, full count per step",
+                    config=dict(workload=WORKLOAD,
                                 kind="langford", n=n, chunk_bits=C, n_moduli=m, parallelism="chunk ranges x%d" % world,
                                 l2="flushed between steps (256 MiB fill); the kernel reads no global memory",
                                 result_check="L(20) = 2,636,337,861,200 reconstructed every run (PAPER.md:380)",
