@@ -41,6 +41,10 @@ WORKLOAD = "L(20): Langford n=20, 2^39 sign vectors (x_1=+1), 2^16 prefix chunks
 # secondary point of the metric (configs[4]): Skolem n = 24, 2^20 chunks, 8 primes + 1 check prime,
 # a fixed seeded 1/64 subset of chunks (256 runs of 64 contiguous chunks)
 WL24 = dict(kind=0, n=24, chunk_bits=20, n_moduli=9, runs=256, run_len=64)
+# BASELINE.json configs[0..3] other than the workload: (kind, n, chunk_bits, moduli incl. check, back-to-back
+# launches timed, printed count: PAPER.md Table 8 :376,:378 / Table 7 :351,:352,:354)
+OTHER_CONFIGS = [(1, 12, 6, 4, 100, 108144), (0, 13, 8, 4, 100, 1520280), (1, 16, 10, 6, 20, 326721800),
+                 (0, 16, 10, 6, 20, 700078384), (0, 21, 18, 7, 1, 61782464083584)]
 SM_COUNT, LANES_PER_SM_CLK = 148, 128
 
 
@@ -364,6 +368,36 @@ def run_gpu(args):
                        terms=terms24, seconds=t24, value=terms24 / t24, unit="terms/s",
                        projected_full_run_s=(1 << 47) / (terms24 / t24))
 
+        # the other BASELINE.json configs (parity-test cases; timed here for SURVEY §8(d)'s per-config table)
+        other = None
+        if not args.no_configs and world == 1 and not args.profile_chunks:
+            other = []
+            for (k2, n2, C2, m2, reps, want) in OTHER_CONFIGS:
+                mod2 = pb.pairings_default_moduli(m2)
+                rows2 = 1 << C2
+                out2 = torch.empty((rows2, m2), dtype=torch.int32, device="cuda")
+                nz2 = torch.zeros(1, dtype=torch.int64, device="cuda")
+                o3 = pb.LaunchOpts(variant=pb.VARIANT_AUTO)
+                o3.nonzero_terms = nz2.data_ptr()
+                pb.count_pairings_ex(k2, n2, C2, 0, rows2, mod2, out2.data_ptr(), stream, o3)    # warm-up + phi
+                torch.cuda.synchronize()
+                flat2 = (ctypes.c_uint32 * (rows2 * m2)).from_buffer_copy(out2.cpu().numpy().tobytes())
+                D2, S2 = pb.pairings_reconstruct(k2, n2, mod2, pb.pairings_sum_rows(flat2, mod2))
+                assert S2 == want, (k2, n2, S2, want)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                for _ in range(reps):
+                    pb.count_pairings_ex(k2, n2, C2, 0, rows2, mod2, out2.data_ptr(), stream, opts)
+                e1.record()
+                torch.cuda.synchronize()
+                sec = e0.elapsed_time(e1) * 1e-3 / reps
+                terms2 = 1 << (2 * n2 - 1)
+                phi2 = float(nz2.item()) / terms2
+                ops2, ys2 = yardstick_ops(k2, n2, m2, phi2)
+                other.append(dict(config="%s(%d)" % (KIND_NAME[k2], n2), chunk_bits=C2, n_moduli=m2, launches_timed=reps,
+                                  seconds_per_count=sec, value=terms2 / sec, unit="terms/s", phi=phi2, ops_per_term=ops2,
+                                  roofline_frac=ops2 * terms2 / sec / peak, identified=S2))
+
         cpu = cpu_baseline(kind, n) if not args.no_cpu else None
         line = dict(metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s", n_gpus=world,
                     steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=dev_ms / args.steps,
@@ -378,7 +412,7 @@ def run_gpu(args):
                              d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps,
                              clocks=clocks_e2e),
                     profile_only=bool(args.profile_chunks),
-                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24, lemma24=lemma24,
+                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24, lemma24=lemma24, other_configs=other,
                     paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")
     if dist is not None:
         dist.barrier()
@@ -396,6 +430,7 @@ def main():
     ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
     ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 256 seeded S(24) runs to time")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-configs", action="store_true", help="skip the timing of the other BASELINE configs")
     ap.add_argument("--profile-chunks", type=int, default=0,
                     help="profiling aid: only the first N chunks per step (short launches for ncu); the line is marked, not a bench value")
     args = ap.parse_args()

@@ -190,13 +190,21 @@ int pairings_lemma24(int kind, int n);
  *   *chunks_needed_out (may be NULL) = number of chunks this mode evaluates in total.
  *   When *chunks_done_out == *chunks_needed_out, total_out holds H mod p_i (symmetry factor applied);
  *   before that it is the raw partial sum.  A journal that already holds chunks of the x_2 = -1 half
- *   (written by a run without the flag) is refused with PAIRINGS_EJOURNAL. */
-enum { PAIRINGS_RUN_LEMMA24 = 1 };
+ *   (written by a run without the flag) is refused with PAIRINGS_EJOURNAL.
+ *
+ * PAIRINGS_RUN_DUPLICATE: the paper's protection against silent GPU errors (every job is run
+ * twice, a third time on disagreement; §8(f) NEXT #3).  Every chunk range is evaluated twice — the second
+ * time with another launch geometry (another Gray-bit count: another thread <-> term mapping and summation
+ * order) — and the rows are compared word by word; on a mismatch a third run decides, and if no two runs
+ * agree the call fails with PAIRINGS_ECHECK.  *duplicate_mismatches_out (may be NULL) counts the ranges
+ * whose first two runs disagreed.  Costs twice the time. */
+enum { PAIRINGS_RUN_LEMMA24 = 1, PAIRINGS_RUN_DUPLICATE = 2 };
 int pairings_run_ex(int kind, int n, int chunk_bits,
                     const uint32_t* moduli, int n_moduli,
                     uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
                     void* stream, const pairings_launch_opts* opts, unsigned flags,
-                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out);
+                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                    uint64_t* duplicate_mismatches_out);
 
 /* §8(a) row a7 — CRT reconstruction ("the actual value is obtained using the chinese
  * remainder theorem") and the exact division of Lemma 2.1.

@@ -9,7 +9,7 @@ from .api import (  # noqa: F401
     count_pairings, count_pairings_ex, count_pairings_host, pairings_has_swar,
     pairings_default_moduli, pairings_min_moduli, pairings_bound_moduli,
     pairings_partition, pairings_rank_range, pairings_sum_rows,
-    pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_lemma24, RUN_LEMMA24,
+    pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_lemma24, RUN_LEMMA24, RUN_DUPLICATE,
     default_chunk_bits, default_chunks_per_call,
     pairings_reconstruct, pairings_crt_signed, pairings_strerror, pairings_build_info,
     pairings_issue_probe,

@@ -26,6 +26,10 @@ def main(argv=None) -> int:
     ap.add_argument("--chunks-per-call", type=int, default=None)
     ap.add_argument("--lemma24", action="store_true",
                     help="symmetry 3 (Lemma 2.4, PAPER.md:215-249): evaluate only the x_2 = +1 half and double it")
+    ap.add_argument("--duplicate", action="store_true",
+                    help="PAPER.md:99: evaluate every chunk range twice (other launch geometry), third run on mismatch")
+    ap.add_argument("--tight-moduli", action="store_true",
+                    help="size the prime set from 2^(2n-1) prod(2n-d_k) instead of (2n)^n 2^(2n)")
     ap.add_argument("--journal", default=None)
     ap.add_argument("--max-calls", type=int, default=0)
     ap.add_argument("--json", action="store_true")
@@ -33,7 +37,8 @@ def main(argv=None) -> int:
 
     kind = api.SKOLEM if a.kind.upper() == "S" else api.LANGFORD
     n = a.n
-    m = a.moduli if a.moduli is not None else api.pairings_bound_moduli(kind, n) + 1
+    m = a.moduli if a.moduli is not None else \
+        (api.pairings_min_moduli(kind, n) if a.tight_moduli else api.pairings_bound_moduli(kind, n)) + 1
     moduli = api.pairings_default_moduli(m)
     C = a.chunk_bits if a.chunk_bits is not None else api.default_chunk_bits(n)
     per_call = a.chunks_per_call if a.chunks_per_call is not None else api.default_chunks_per_call(n, C)
@@ -42,10 +47,12 @@ def main(argv=None) -> int:
     init_s = time.perf_counter() - ti
     t0 = time.perf_counter()
     total, done, needed = api.pairings_run_ex(kind, n, C, moduli, per_call, a.journal, a.max_calls, 0, None,
-                                              api.RUN_LEMMA24 if a.lemma24 else 0)
+                                              (api.RUN_LEMMA24 if a.lemma24 else 0) |
+                                              (api.RUN_DUPLICATE if a.duplicate else 0))
     dt = time.perf_counter() - t0
     res = dict(kind=a.kind.upper(), n=n, chunk_bits=C, moduli=moduli, chunks_done=done, chunks_needed=needed,
-               chunks=1 << C, lemma24=bool(a.lemma24), seconds=dt, init_seconds=init_s, total_residues=total)
+               chunks=1 << C, lemma24=bool(a.lemma24), duplicate=bool(a.duplicate),
+               duplicate_mismatches=api.pairings_run_ex.last_mismatches, seconds=dt, init_seconds=init_s, total_residues=total)
     if done == needed:
         D, S = api.pairings_reconstruct(kind, n, moduli, total)
         evaluated = needed << (2 * n - 1 - C)

@@ -60,7 +60,7 @@ def lib():
         "pairings_journal_append": (i, [cp, i, i, i, u32p, i, u64, u64, u32p]),
         "pairings_journal_load": (ctypes.c_int64, [cp, i, i, i, u32p, i, u64p, ctypes.c_int64, u32p]),
         "pairings_run": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, u32p, u64p]),
-        "pairings_run_ex": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, ctypes.c_uint, u32p, u64p, u64p]),
+        "pairings_run_ex": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, ctypes.c_uint, u32p, u64p, u64p, u64p]),
         "pairings_lemma24": (i, [i, i]),
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
@@ -202,7 +202,7 @@ def pairings_run(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=None
     return [int(t[j]) for j in range(k)], int(done.value)
 
 
-RUN_LEMMA24 = 1
+RUN_LEMMA24, RUN_DUPLICATE = 1, 2
 
 
 def pairings_lemma24(kind: int, n: int) -> int:
@@ -212,14 +212,16 @@ def pairings_lemma24(kind: int, n: int) -> int:
 
 def pairings_run_ex(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=None, max_calls=0, stream: int = 0,
                     opts: Optional[LaunchOpts] = None, flags: int = 0):
-    """Whole-job host driver with flags.  Returns (total residues, chunks done, chunks needed)."""
+    """Whole-job host driver with flags.  Returns (total residues, chunks done, chunks needed); the number of
+    duplicate-run mismatches of the last call is kept in pairings_run_ex.last_mismatches."""
     k = len(moduli)
     t = _u32([0] * k)
-    done, needed = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    done, needed, mism = ctypes.c_uint64(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
     jp = os.fsencode(journal_path) if journal_path is not None else None
     _check(lib().pairings_run_ex(kind, n, chunk_bits, _u32(moduli), k, chunks_per_call, jp, max_calls,
                                  ctypes.c_void_p(stream), _opts(opts), flags, t, ctypes.byref(done),
-                                 ctypes.byref(needed)), "pairings_run_ex")
+                                 ctypes.byref(needed), ctypes.byref(mism)), "pairings_run_ex")
+    pairings_run_ex.last_mismatches = int(mism.value)
     return [int(t[j]) for j in range(k)], int(done.value), int(needed.value)
 
 
@@ -257,16 +259,16 @@ def default_chunks_per_call(n: int, chunk_bits: int) -> int:
 
 def count(kind: int, n: int, chunk_bits: Optional[int] = None, n_moduli: Optional[int] = None,
           chunks_per_call: Optional[int] = None, journal_path=None, opts: Optional[LaunchOpts] = None,
-          lemma24: bool = False):
+          lemma24: bool = False, duplicate: bool = False, tight_moduli: bool = False):
     """Convenience: the whole path for (kind, n) -> (D, S).  Calls only the C ABI."""
-    if n_moduli is None:
-        n_moduli = pairings_bound_moduli(kind, n) + 1
+    if n_moduli is None:      # §8(f) NEXT #2: the tight bound 2^{2n-1} prod(2n-d_k) instead of north_star's (2n)^n 2^{2n}
+        n_moduli = (pairings_min_moduli(kind, n) if tight_moduli else pairings_bound_moduli(kind, n)) + 1
     moduli = pairings_default_moduli(n_moduli)
     if chunk_bits is None:
         chunk_bits = default_chunk_bits(n)
     if chunks_per_call is None:
         chunks_per_call = default_chunks_per_call(n, chunk_bits)
     total, done, needed = pairings_run_ex(kind, n, chunk_bits, moduli, chunks_per_call, journal_path, 0, 0, opts,
-                                          RUN_LEMMA24 if lemma24 else 0)
+                                          (RUN_LEMMA24 if lemma24 else 0) | (RUN_DUPLICATE if duplicate else 0))
     assert done == needed
     return pairings_reconstruct(kind, n, moduli, total)

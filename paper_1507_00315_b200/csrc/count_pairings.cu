@@ -308,13 +308,15 @@ int count_pairings_host(int kind, int n, int chunk_bits, uint64_t chunk_begin, u
 int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
                     uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
                     void* stream, const pairings_launch_opts* opts, unsigned flags,
-                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out) {
+                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                    uint64_t* duplicate_mismatches_out) {
     int rc = validate(kind, n, chunk_bits, 0, 0, moduli, n_moduli, total_out); if (rc) return rc;
     if (!total_out || !chunks_done_out) return PAIRINGS_ENULL;
     if (chunks_per_call == 0) return PAIRINGS_EINVAL_CHUNK;
-    if (flags & ~(unsigned)PAIRINGS_RUN_LEMMA24) return PAIRINGS_EINVAL_OPTS;
+    if (flags & ~(unsigned)(PAIRINGS_RUN_LEMMA24 | PAIRINGS_RUN_DUPLICATE)) return PAIRINGS_EINVAL_OPTS;
     for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
     *chunks_done_out = 0;
+    if (duplicate_mismatches_out) *duplicate_mismatches_out = 0;
 
     // Lemma 2.4: negating the even positions maps the x_2 = +1 half of every
     // sum onto the x_2 = -1 half, term for term (up to the sign pairings_lemma24 reports).  The most
@@ -353,7 +355,7 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
     need = pairings_partition(chunk_bits, chunks_per_call, done.data(), (int)(done.size() / 2), ranges.data(), need);
     if (need < 0) return (int)need;
 
-    std::vector<uint32_t> rows;
+    std::vector<uint32_t> rows, rows_dup;
     int64_t calls = 0;
     for (int64_t r = 0; r < need; r++) {
         if (max_calls > 0 && calls >= max_calls) break;
@@ -361,6 +363,34 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
         rows.resize((size_t)(e - b) * (size_t)n_moduli);
         rc = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, rows.data(), stream, opts);
         if (rc) return rc;
+        if (flags & PAIRINGS_RUN_DUPLICATE) {
+            // "every GPU job run twice ... a third run on mismatch" (silent GPU errors).  With one
+            // GPU the second run uses another launch geometry (other Gray-bit count: other thread <-> term
+            // mapping, other summation order), so a repeatable fault of one mapping does not hide itself.
+            Geometry geo; rc = choose_geometry(kind, n, chunk_bits, e - b, opts, &geo); if (rc) return rc;
+            pairings_launch_opts alt; std::memset(&alt, 0, sizeof alt);
+            alt.variant = geo.variant;
+            auto rerun = [&](int first_dg, std::vector<uint32_t>& dst) -> int {
+                dst.resize(rows.size());
+                int rc2 = PAIRINGS_EINVAL_OPTS;
+                for (int dg = first_dg; dg <= first_dg + 4 && rc2 == PAIRINGS_EINVAL_OPTS; dg += 2) {   // nearest admissible g
+                    alt.gray_bits = geo.g - dg > 0 ? geo.g - dg : geo.g + dg;
+                    rc2 = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, dst.data(), stream, &alt);
+                }
+                if (rc2 == PAIRINGS_EINVAL_OPTS)                      // no other geometry exists (tiny jobs): the same one again
+                    rc2 = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, dst.data(), stream, opts);
+                return rc2;
+            };
+            rc = rerun(1, rows_dup); if (rc) return rc;
+            if (std::memcmp(rows.data(), rows_dup.data(), rows.size() * sizeof(uint32_t)) != 0) {
+                if (duplicate_mismatches_out) ++*duplicate_mismatches_out;
+                std::vector<uint32_t> third;
+                rc = rerun(2, third); if (rc) return rc;
+                if (std::memcmp(third.data(), rows.data(), rows.size() * sizeof(uint32_t)) == 0) { /* first run stands */ }
+                else if (std::memcmp(third.data(), rows_dup.data(), rows.size() * sizeof(uint32_t)) == 0) rows.swap(rows_dup);
+                else return PAIRINGS_ECHECK;                          // three runs, no two agree
+            }
+        }
         uint32_t row_sum[PAIRINGS_MAX_MODULI] = {0};
         rc = pairings_sum_rows(rows.data(), e - b, moduli, n_moduli, row_sum); if (rc) return rc;
         if (journal_path) {
@@ -382,7 +412,7 @@ int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_
                  void* stream, const pairings_launch_opts* opts,
                  uint32_t* total_out, uint64_t* chunks_done_out) {
     return pairings_run_ex(kind, n, chunk_bits, moduli, n_moduli, chunks_per_call, journal_path, max_calls,
-                           stream, opts, 0u, total_out, chunks_done_out, nullptr);
+                           stream, opts, 0u, total_out, chunks_done_out, nullptr, nullptr);
 }
 
 const char* pairings_build_info(void) {

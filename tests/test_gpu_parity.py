@@ -262,3 +262,16 @@ def test_full_totals_match_the_paper(kind, n, C, paper_counts):
     assert Sid == paper_counts[(kind, n)] and D == 2 * Sid
     # and with symmetry 3: half the work
     assert pb.count(kind, n, lemma24=True) == (D, Sid)
+
+
+@pytest.mark.parametrize("kind,n,C", [(L, 12, 6), (S, 13, 8), (L, 8, 3), (S, 16, 10)])
+def test_duplicate_run_mode_and_tight_moduli(kind, n, C, paper_counts):
+    # §8(f) NEXT #3 (every job twice, third run on mismatch) and NEXT #2 (tight prime budget)
+    moduli = pb.pairings_default_moduli(pb.pairings_min_moduli(kind, n) + 1)
+    assert len(moduli) <= pb.pairings_bound_moduli(kind, n) + 1
+    total, done, needed = pb.pairings_run_ex(kind, n, C, moduli, 1 << max(C - 2, 0), None, 0, 0, None,
+                                             pb.RUN_DUPLICATE | pb.RUN_LEMMA24)
+    assert done == needed == 1 << (C - 1) and pb.pairings_run_ex.last_mismatches == 0
+    D, Sid = pb.pairings_reconstruct(kind, n, moduli, total)
+    assert Sid == paper_counts[(kind, n)] and D == 2 * Sid
+    assert pb.count(kind, n, duplicate=True, tight_moduli=True) == (D, Sid)

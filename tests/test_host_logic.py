@@ -260,4 +260,4 @@ def test_run_ex_without_pairings_needs_no_gpu():
     assert (total, done, needed) == ([0, 0, 0, 0], 0, 0)
     assert pb.pairings_reconstruct(pb.SKOLEM, 10, moduli, total) == (0, 0)
     with pytest.raises(pb.PairingsError):
-        pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, 2)      # unknown flag
+        pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, 4)      # unknown flag
