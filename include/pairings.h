@@ -226,6 +226,41 @@ int pairings_reconstruct(int kind, int n,
 int pairings_crt_signed(const uint32_t* moduli, int n_moduli, const uint32_t* residues,
                         char* out_dec, size_t cap);
 
+/* ------------------------------------------------------------------------------------------------
+ * Approximate counting by parallel tempering — PAPER.md §3 (:259-325), Algorithm 2 (:291-319);
+ * SURVEY.md §8(f) NEXT #4.  A second, statistical workload beside the exact count.
+ *
+ * The system: colour k occupies bins a_k and a_k + d_k, a_k in [1, 2n - d_k]; the energy of
+ * a configuration is its number of empty bins; Z(0) = prod_k (2n - d_k) = (2n-1)!/(n-1)! for Skolem, and the
+ * E = 0 configurations are the pairings (reflections distinct).  Levels: betas[0] = 0 < betas[1] < ... (HOST,
+ * n_levels <= PAIRINGS_PT_MAX_LEVELS), the level above the last one is beta = infinity (reading C1).
+ *
+ * pairings_pt_run enqueues replicas [replica_begin, replica_end) of Algorithm 2, `iterations` iterations each
+ * of which the first `burn_in` (< iterations) are run but not counted (0 = as printed; reading C4: many short
+ * replicas need it, a replica started from a random configuration is biased by O(relaxation time / iterations)),
+ * one thread per replica, and ADDS to the DEVICE counters (the caller zeroes them):
+ *     hist_dev   n_levels x (2n+1) uint64: hist[j][E] = samples of level j with E empty bins
+ *     moves_dev  n_levels uint64: accepted moves of level j         (column W1 of Table 6)
+ *     swaps_dev  n_levels uint64: accepted exchanges j <-> j+1      (column W2)
+ * Random numbers: draw(seed, ctr) = splitmix64_mix(seed + 0x9E3779B97F4A7C15 (ctr + 1)), counter layout and
+ * the integer decision rule "u < floor(p 2^32)" as in DESIGN.md (readings C2, C3): the counters depend only on
+ * (kind, n, betas, replica range, iterations, seed) — not on the launch — and add up over disjoint replica
+ * ranges, which is how the work is sharded over calls or GPUs.  iterations <= 2^25, replica_end <= 2^30.
+ * Invalid arguments are reported before anything is enqueued; the call synchronises the stream once (the
+ * threshold table is staged from host memory) and then returns with the kernel enqueued. */
+#define PAIRINGS_PT_MAX_LEVELS 32
+int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
+                    uint64_t replica_begin, uint64_t replica_end, uint64_t iterations, uint64_t burn_in, uint64_t seed,
+                    uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream);
+
+/* Host: Ratio(j)/iterations of Algorithm 2 from the histogram (HOST, n_levels x (2n+1)),
+ *     ratios_out[j] = sum_E hist[j][E] exp(-(beta(j+1) - beta(j)) E) / sum_E hist[j][E]     (last level: [E = 0]),
+ * and *log_distinct_out = log( Z(0) prod_j ratios[j] ), the natural logarithm of the estimated number of
+ * pairings with reflections distinct (halve for the paper's S(n) / L(n), Table 6 caption).
+ * PAIRINGS_ERANGE if a level has no samples or a ratio is estimated as zero. */
+int pairings_pt_estimate(int kind, int n, const double* betas, int n_levels, const uint64_t* hist_host,
+                         double* ratios_out, double* log_distinct_out);
+
 /* Measurement helper (not on the path): enqueues an integer-issue calibration kernel — independent
  * chains (ILP 8) of mode 0: IADD3, 1: LOP3, 2: IMAD, 3: IADD3:IMAD 1:1 — and reports how many
  * thread-instructions of that class it executes, for the roofline denominator.

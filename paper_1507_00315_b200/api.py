@@ -64,6 +64,9 @@ def lib():
         "pairings_lemma24": (i, [i, i]),
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
+        "pairings_pt_run": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64, u64, u64, u64, u64, vp, vp, vp, vp]),
+        "pairings_pt_estimate": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64p, ctypes.POINTER(ctypes.c_double),
+                                     ctypes.POINTER(ctypes.c_double)]),
         "pairings_issue_probe": (i, [i, i, i, i, vp, vp, u64p]),
         "pairings_strerror": (cp, [i]),
         "pairings_build_info": (cp, []),
@@ -245,6 +248,27 @@ def pairings_issue_probe(mode: int, blocks: int, threads: int, iters: int, out_d
     _check(lib().pairings_issue_probe(mode, blocks, threads, iters, ctypes.c_void_p(out_dev_ptr),
                                       ctypes.c_void_p(stream), ctypes.byref(cnt)), "pairings_issue_probe")
     return int(cnt.value)
+
+
+def pairings_pt_run(kind, n, betas, replica_begin, replica_end, iterations, burn_in, seed, hist_dev_ptr: int,
+                    moves_dev_ptr: int, swaps_dev_ptr: int, stream: int = 0):
+    """Approximate counter (Algorithm 2): ADDS to the DEVICE counters hist (levels x (2n+1)
+    uint64), moves and swaps (levels uint64 each)."""
+    b = (ctypes.c_double * len(betas))(*betas)
+    _check(lib().pairings_pt_run(kind, n, b, len(betas), replica_begin, replica_end, iterations, burn_in, seed,
+                                 ctypes.c_void_p(hist_dev_ptr), ctypes.c_void_p(moves_dev_ptr),
+                                 ctypes.c_void_p(swaps_dev_ptr), ctypes.c_void_p(stream)), "pairings_pt_run")
+
+
+def pairings_pt_estimate(kind, n, betas, hist):
+    """hist: levels x (2n+1) counts.  Returns (ratios per level, log of the estimated reflections-distinct count)."""
+    M = len(betas)
+    b = (ctypes.c_double * M)(*betas)
+    flat = (ctypes.c_uint64 * (M * (2 * n + 1)))(*[int(v) for row in hist for v in row])
+    r = (ctypes.c_double * M)()
+    lz = ctypes.c_double(0.0)
+    _check(lib().pairings_pt_estimate(kind, n, b, M, flat, r, ctypes.byref(lz)), "pairings_pt_estimate")
+    return [float(v) for v in r], float(lz.value)
 
 
 def default_chunk_bits(n: int) -> int:

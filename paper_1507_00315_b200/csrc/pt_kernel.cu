@@ -1,0 +1,228 @@
+// Approximate counting by parallel tempering (§3, :259-325; Algorithm 2, :291-319) —
+// SURVEY.md §8(f) NEXT #4, a second workload beside the exact count.
+//
+// One thread runs one replica of Algorithm 2: M configurations (one per inverse temperature), per
+// iteration (in the paper's order) the ratio sample of every level, one Metropolis move per level,
+// then the exchanges of neighbouring levels j = 1..M-1 in sequence.  Replicas are independent, so a
+// launch is embarrassingly parallel; what comes back is integer only:
+//     hist[j][E]  how often level j was seen with E empty bins  (Ratio(j) = sum_E hist[j][E] w_j(E), host)
+//     moves[j], swaps[j]  accepted moves / exchanges (the W1, W2 columns of Table 6)
+// Every random decision is "u < threshold" on 32-bit integers, the thresholds floor(p 2^32) are computed
+// once on the host, and the generator is counter-based (readings C1-C3 in DESIGN.md), so the counters
+// are reproducible bit for bit — that is what the parity tests compare with the oracle.
+//
+// State of a replica lives in shared memory, byte-interleaved over the block's threads:
+//   pos[slot][k]   position a_k of colour k (bins a_k and a_k + d_k)            M x n bytes
+//   occ[slot][b]   balls in bin b                                                M x (2n+1) bytes
+//   lev[j] = slot holding level j's configuration, E[j] its energy               2 M bytes
+// An exchange swaps lev / E entries, not configurations.  The energy change of a move is counted
+// incrementally: bins that become empty minus bins that become occupied.
+#include "pairings.h"
+#include "internal.h"
+
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace pairings {
+
+constexpr int PT_THREADS = 64;
+
+struct PtParams {
+    int kind, n, M;
+    uint64_t replica_begin, replica_end, iterations, burn_in, seed;
+    const uint64_t* move_thr;    // DEVICE, M x 2: threshold for dE = 1, 2
+    const uint64_t* swap_thr;    // DEVICE, (M-1) x (2n+1): threshold for dE = E_j - E_{j+1} > 0
+    unsigned long long *hist, *moves, *swaps;   // DEVICE
+};
+
+__device__ __forceinline__ uint64_t pt_mix64(uint64_t z) {
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ULL;
+    z ^= z >> 27; z *= 0x94D049BB133111EBULL;
+    z ^= z >> 31;
+    return z;
+}
+__device__ __forceinline__ uint64_t pt_draw(uint64_t seed, uint64_t ctr) {
+    return pt_mix64(seed + 0x9E3779B97F4A7C15ULL * (ctr + 1));
+}
+
+__global__ void __launch_bounds__(PT_THREADS) pt_kernel(const PtParams p) {
+    extern __shared__ unsigned char smem_raw[];
+    const int n = p.n, N = 2 * n, M = p.M, kind = p.kind;
+    const int tid = threadIdx.x, BD = PT_THREADS;
+    // block counters first (32-bit, flushed at the end), then the byte-interleaved replica state
+    unsigned int* shist = reinterpret_cast<unsigned int*>(smem_raw);           // M x (N+1)
+    unsigned int* smoves = shist + M * (N + 1);                                 // M
+    unsigned int* sswaps = smoves + M;                                          // M
+    unsigned char* st = reinterpret_cast<unsigned char*>(sswaps + M);
+    const int POS = 0, OCC = M * n, LEV = OCC + M * (N + 1), EN = LEV + M;      // byte offsets of the per-thread state
+#define ST(i) st[(i) * BD + tid]
+    for (int i = tid; i < M * (N + 1) + 2 * M; i += BD) shist[i] = 0;
+    __syncthreads();
+
+    const uint64_t r = p.replica_begin + (uint64_t)blockIdx.x * BD + tid;
+    const bool active = r < p.replica_end;
+    const uint64_t S = n > 3 ? n : 3, T = p.iterations, seed = p.seed;
+
+    if (active) {
+        // ---- "C(i) <- a random configuration"
+        for (int j = 0; j < M; j++) {
+            for (int b = 0; b <= N; b++) ST(OCC + j * (N + 1) + b) = 0;
+            for (int k = 1; k <= n; k++) {
+                const int d = dist(kind, k);
+                const uint64_t u = pt_draw(seed, ((r * (T + 1)) * M + j) * S + (k - 1)) >> 32;
+                const int a = 1 + (int)((u * (uint64_t)(N - d)) >> 32);
+                ST(POS + j * n + (k - 1)) = (unsigned char)a;
+                ST(OCC + j * (N + 1) + a) += 1;
+                ST(OCC + j * (N + 1) + a + d) += 1;
+            }
+            int e = 0;
+            for (int b = 1; b <= N; b++) e += (ST(OCC + j * (N + 1) + b) == 0);
+            ST(LEV + j) = (unsigned char)j;
+            ST(EN + j) = (unsigned char)e;
+        }
+        for (uint64_t t = 0; t < T; t++) {
+            const uint64_t base = (r * (T + 1) + (t + 1)) * M;
+            // ---- step 1: ratio samples
+            const bool counted = t >= p.burn_in;
+            if (counted) for (int j = 0; j < M; j++) atomicAdd(&shist[j * (N + 1) + ST(EN + j)], 1u);
+            // ---- step 2: one move per level
+            for (int j = 0; j < M; j++) {
+                const int slot = ST(LEV + j);
+                const uint64_t w = pt_draw(seed, (base + j) * S + 0);
+                const int k = 1 + (int)(((w & 0xFFFFFFFFULL) * (uint64_t)n) >> 32);
+                const int d = dist(kind, k);
+                const int a1 = 1 + (int)(((w >> 32) * (uint64_t)(N - d)) >> 32);
+                const int a0 = ST(POS + slot * n + (k - 1));
+                const int ob = OCC + slot * (N + 1);
+                int dE = 0;
+                unsigned char c;
+                c = ST(ob + a0) - 1; ST(ob + a0) = c; dE += (c == 0);
+                c = ST(ob + a0 + d) - 1; ST(ob + a0 + d) = c; dE += (c == 0);
+                c = ST(ob + a1) + 1; ST(ob + a1) = c; dE -= (c == 1);
+                c = ST(ob + a1 + d) + 1; ST(ob + a1 + d) = c; dE -= (c == 1);
+                bool accept = dE <= 0;
+                if (!accept) {
+                    const uint64_t u = pt_draw(seed, (base + j) * S + 1) >> 32;
+                    accept = u < p.move_thr[j * 2 + (dE - 1)];
+                }
+                if (accept) {
+                    ST(POS + slot * n + (k - 1)) = (unsigned char)a1;
+                    ST(EN + j) = (unsigned char)((int)ST(EN + j) + dE);
+                    if (counted) atomicAdd(&smoves[j], 1u);
+                } else {
+                    ST(ob + a1) -= 1; ST(ob + a1 + d) -= 1; ST(ob + a0) += 1; ST(ob + a0 + d) += 1;
+                }
+            }
+            // ---- step 3: exchanges j, j+1 in sequence
+            for (int j = 0; j + 1 < M; j++) {
+                const int e0 = ST(EN + j), e1 = ST(EN + j + 1), dE = e0 - e1;
+                bool accept = dE <= 0;
+                if (!accept) {
+                    const uint64_t u = pt_draw(seed, (base + j) * S + 2) >> 32;
+                    accept = u < p.swap_thr[j * (N + 1) + dE];
+                }
+                if (accept) {
+                    const unsigned char l0 = ST(LEV + j);
+                    ST(LEV + j) = ST(LEV + j + 1); ST(LEV + j + 1) = l0;
+                    ST(EN + j) = (unsigned char)e1; ST(EN + j + 1) = (unsigned char)e0;
+                    if (counted) atomicAdd(&sswaps[j], 1u);
+                }
+            }
+        }
+    }
+#undef ST
+    __syncthreads();
+    for (int i = tid; i < M * (N + 1); i += BD) if (shist[i]) atomicAdd(&p.hist[i], (unsigned long long)shist[i]);
+    for (int i = tid; i < M; i += BD) {
+        if (smoves[i]) atomicAdd(&p.moves[i], (unsigned long long)smoves[i]);
+        if (sswaps[i]) atomicAdd(&p.swaps[i], (unsigned long long)sswaps[i]);
+    }
+}
+
+static uint64_t pt_threshold(double prob) {
+    if (prob >= 1.0) return 1ULL << 32;
+    return (uint64_t)std::floor(prob * 4294967296.0);
+}
+
+static int pt_check(int kind, int n, const double* betas, int n_levels) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    if (!betas) return PAIRINGS_ENULL;
+    if (n_levels < 1 || n_levels > PAIRINGS_PT_MAX_LEVELS) return PAIRINGS_EINVAL_OPTS;
+    if (betas[0] != 0.0) return PAIRINGS_EINVAL_OPTS;                 // Z(0) is the closed form the estimate starts from
+    for (int j = 1; j < n_levels; j++) if (!(betas[j] > betas[j - 1]) || !std::isfinite(betas[j])) return PAIRINGS_EINVAL_OPTS;
+    return PAIRINGS_OK;
+}
+
+}  // namespace pairings
+
+using namespace pairings;
+
+extern "C" {
+
+int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
+                    uint64_t replica_begin, uint64_t replica_end, uint64_t iterations, uint64_t burn_in, uint64_t seed,
+                    uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream) {
+    int rc = pt_check(kind, n, betas, n_levels); if (rc) return rc;
+    if (replica_begin > replica_end || iterations == 0 || iterations > (1ULL << 25) || burn_in >= iterations) return PAIRINGS_EINVAL_OPTS;
+    if (replica_end > (1ULL << 30)) return PAIRINGS_EINVAL_OPTS;      // the draw counter must stay below 2^64
+    if (!hist_dev || !moves_dev || !swaps_dev) return PAIRINGS_ENULL;
+    if (replica_begin == replica_end) return PAIRINGS_OK;
+    const int M = n_levels, N = 2 * n;
+    std::vector<uint64_t> thr((size_t)(M * 2 + M * (N + 1)), 0);
+    for (int j = 0; j < M; j++)
+        for (int dE = 1; dE <= 2; dE++) thr[(size_t)(j * 2 + dE - 1)] = pt_threshold(std::exp(-betas[j] * (double)dE));
+    for (int j = 0; j + 1 < M; j++)
+        for (int dE = 1; dE <= N; dE++)
+            thr[(size_t)(M * 2 + j * (N + 1) + dE)] = pt_threshold(std::exp(-(betas[j + 1] - betas[j]) * (double)dE));
+
+    cudaStream_t s = (cudaStream_t)stream;
+    (void)cudaGetLastError();
+    uint64_t* dthr = nullptr;
+    if (cudaMallocAsync((void**)&dthr, thr.size() * sizeof(uint64_t), s) != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    cudaError_t e = cudaMemcpyAsync(dthr, thr.data(), thr.size() * sizeof(uint64_t), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);               // thr is a local: the copy must have left it
+    PtParams p; std::memset(&p, 0, sizeof p);
+    p.kind = kind; p.n = n; p.M = M;
+    p.replica_begin = replica_begin; p.replica_end = replica_end; p.iterations = iterations; p.burn_in = burn_in; p.seed = seed;
+    p.move_thr = dthr; p.swap_thr = dthr + M * 2;
+    p.hist = (unsigned long long*)hist_dev; p.moves = (unsigned long long*)moves_dev; p.swaps = (unsigned long long*)swaps_dev;
+    const size_t smem = (size_t)(M * (N + 1) + 2 * M) * sizeof(unsigned int)
+                      + (size_t)PT_THREADS * (size_t)(M * n + M * (N + 1) + 2 * M);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(pt_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) {
+        const uint64_t blocks = (replica_end - replica_begin + PT_THREADS - 1) / PT_THREADS;
+        pt_kernel<<<(unsigned)blocks, PT_THREADS, smem, s>>>(p);
+        e = cudaGetLastError();
+    }
+    cudaError_t e2 = cudaFreeAsync(dthr, s);
+    if (e != cudaSuccess || e2 != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    return PAIRINGS_OK;
+}
+
+int pairings_pt_estimate(int kind, int n, const double* betas, int n_levels, const uint64_t* hist_host,
+                         double* ratios_out, double* log_distinct_out) {
+    int rc = pt_check(kind, n, betas, n_levels); if (rc) return rc;
+    if (!hist_host || !ratios_out || !log_distinct_out) return PAIRINGS_ENULL;
+    const int N = 2 * n;
+    double logz = 0.0;                                                  // log Z(0) = sum_k log(2n - d_k)
+    for (int k = 1; k <= n; k++) logz += std::log((double)(N - dist(kind, k)));
+    for (int j = 0; j < n_levels; j++) {
+        long double num = 0, den = 0;
+        for (int E = 0; E <= N; E++) {
+            const long double h = (long double)hist_host[(size_t)j * (N + 1) + E];
+            den += h;
+            if (j + 1 < n_levels) num += h * (long double)std::exp(-(betas[j + 1] - betas[j]) * (double)E);
+            else if (E == 0) num += h;                                  // beta(M+1) = infinity
+        }
+        if (den == 0 || num == 0) return PAIRINGS_ERANGE;               // no samples, or a ratio estimated as zero
+        ratios_out[j] = (double)(num / den);
+        logz += std::log(ratios_out[j]);
+    }
+    *log_distinct_out = logz;
+    return PAIRINGS_OK;
+}
+
+}  // extern "C"
