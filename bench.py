@@ -45,6 +45,7 @@ WL24 = dict(kind=0, n=24, chunk_bits=20, n_moduli=9, runs=256, run_len=64)
 # launches timed, printed count: PAPER.md Table 8 :376,:378 / Table 7 :351,:352,:354)
 OTHER_CONFIGS = [(1, 12, 6, 4, 100, 108144), (0, 13, 8, 4, 100, 1520280), (1, 16, 10, 6, 20, 326721800),
                  (0, 16, 10, 6, 20, 700078384), (0, 21, 18, 7, 1, 61782464083584)]
+PT_BETAS = [0, 0.54, 1.1, 1.69, 2.33, 3, 3.73, 4.65, 5.82, 8.1, 16, 32]     # PAPER.md:329-341 (Table 6, column beta)
 SM_COUNT, LANES_PER_SM_CLK = 148, 128
 
 
@@ -398,6 +399,36 @@ def run_gpu(args):
                                   seconds_per_count=sec, value=terms2 / sec, unit="terms/s", phi=phi2, ops_per_term=ops2,
                                   roofline_frac=ops2 * terms2 / sec / peak, identified=S2))
 
+        # second workload: the approximate counter, S(12) with the ladder of Table 6
+        ptres = None
+        if not args.no_pt and world == 1 and not args.profile_chunks:
+            import math
+            R, T, burn = 1 << 17, 1 << 11, 0                      # throughput run (too short per replica for an estimate)
+            Mlev = len(PT_BETAS)
+            h = torch.zeros((Mlev, 25), dtype=torch.int64, device="cuda")
+            mv = torch.zeros(Mlev, dtype=torch.int64, device="cuda")
+            sw = torch.zeros(Mlev, dtype=torch.int64, device="cuda")
+            pb.pairings_pt_run(0, 12, PT_BETAS, 0, 1 << 10, 1 << 10, 0, 1, h.data_ptr(), mv.data_ptr(), sw.data_ptr(), stream)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            pb.pairings_pt_run(0, 12, PT_BETAS, 0, R, T, burn, 150700315, h.data_ptr(), mv.data_ptr(), sw.data_ptr(), stream)
+            e1.record()
+            torch.cuda.synchronize()
+            sec = e0.elapsed_time(e1) * 1e-3
+            # estimate run: fewer, longer replicas with burn-in (the cold levels need ~10^4 iterations to relax)
+            h.zero_(); mv.zero_(); sw.zero_()
+            t0 = time.perf_counter()
+            pb.pairings_pt_run(0, 12, PT_BETAS, 0, 1 << 12, 1 << 15, 1 << 14, 150700315, h.data_ptr(), mv.data_ptr(), sw.data_ptr(), stream)
+            torch.cuda.synchronize()
+            est_s = time.perf_counter() - t0
+            ratios, logz = pb.pairings_pt_estimate(0, 12, PT_BETAS, h.cpu().tolist())
+            est = math.exp(logz) / 2
+            ptres = dict(workload="approximate count of S(12), 12 levels (Table 6 ladder, PAPER.md:327-342)",
+                         replicas=R, iterations=T, seconds=sec, metropolis_moves_per_s=R * T * Mlev / sec,
+                         estimate=dict(replicas=1 << 12, iterations=1 << 15, burn_in=1 << 14, seconds=est_s,
+                                       s12_estimate=est, exact=227968, rel_error=est / 227968 - 1))
+
         cpu = cpu_baseline(kind, n) if not args.no_cpu else None
         line = dict(metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s", n_gpus=world,
                     steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=dev_ms / args.steps,
@@ -412,7 +443,7 @@ def run_gpu(args):
                              d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps,
                              clocks=clocks_e2e),
                     profile_only=bool(args.profile_chunks),
-                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24, lemma24=lemma24, other_configs=other,
+                    gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24, lemma24=lemma24, other_configs=other, pt=ptres,
                     paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")
     if dist is not None:
         dist.barrier()
@@ -430,6 +461,7 @@ def main():
     ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
     ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 256 seeded S(24) runs to time")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--no-pt", action="store_true", help="skip the approximate-counter (parallel tempering) measurement")
     ap.add_argument("--no-configs", action="store_true", help="skip the timing of the other BASELINE configs")
     ap.add_argument("--profile-chunks", type=int, default=0,
                     help="profiling aid: only the first N chunks per step (short launches for ncu); the line is marked, not a bench value")
