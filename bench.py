@@ -7,8 +7,11 @@ A "step" is one pass of the whole hot path over the workload: partition -> count
 Gray-code kernel over every chunk of this rank's range) -> rows D2H -> row sums -> (rank 0, after
 the exchange of the per-rank sums) CRT + exact division, checked against the paper's printed count.
 Workload at every N: Langford L(20) — 2^39 sign vectors (x_1 = +1), 2^16 prefix chunks, 6 CRT primes
-+ 1 check prime (BASELINE.json configs[3], the n = 20 point the metric is quoted on).  For N > 1 the
-2^16 chunks are dealt out as contiguous ranges (pairings_rank_range), total work fixed: "strong".
++ 1 check prime (BASELINE.json configs[3], the n = 20 point the metric is quoted on).  For N > 1 the path shards
+by chunk ranges with no data-path collective; the default (`--scaling weak`) keeps the per-GPU work fixed: every
+rank evaluates a whole L(20) pass and rank 0 checks that all ranks' residue sums agree (the paper's duplicate-run
+protocol, one copy per GPU); `--scaling strong` deals the 2^16 chunks out as contiguous ranges
+(pairings_rank_range), total work fixed.
 
 `value`   = terms/s with the rows left in HBM (CUDA events around the kernel launches of a step).
 `e2e`     = terms/s through count_pairings_host (HOST output buffer; allocation, launch, D2H copy
@@ -135,7 +138,7 @@ def run_reference(args):
     sample = "%d seeded chunks of 2^17 sign vectors of L(20) per step on %d threads" % (per_step, threads)
     line = dict(impl="reference", metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s",
                 n_gpus=args.gpus, steps=steps, warmup=warm, ms_per_step=1e3 * t_total / steps,
-                higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
+                higher_is_better=True, scaling=args.scaling, vs_baseline=None, dtype="int32", data="synthetic",
                 config=dict(workload=WORKLOAD, kind="langford", n=n, chunk_bits=WL["chunk_bits"], n_moduli=WL["n_moduli"],
                             sample="each step is a bounded sample of the workload: " + sample),
                 cpu_baseline=dict(value=value, unit="terms/s", cores=threads, kind="oracle", sample=sample),
@@ -213,12 +216,13 @@ def run_gpu(args):
 
     kind, n, C, m = WL["kind"], WL["n"], WL["chunk_bits"], WL["n_moduli"]
     moduli = pb.pairings_default_moduli(m)
-    begin, end = pb.pairings_rank_range(C, rank, world)
+    weak = args.scaling == "weak"
+    begin, end = (0, 1 << C) if weak else pb.pairings_rank_range(C, rank, world)
     if args.profile_chunks:                      # short launches for ncu captures; not a bench value
         end = min(end, begin + args.profile_chunks)
     rows = end - begin
     terms_rank = rows << (2 * n - 1 - C)
-    terms_job = (1 << (2 * n - 1)) if not args.profile_chunks else terms_rank * world
+    terms_job = terms_rank * world if (weak or args.profile_chunks) else (1 << (2 * n - 1))
     stream = torch.cuda.current_stream().cuda_stream
     out = torch.empty((rows, m), dtype=torch.int32, device="cuda")
     host_rows = torch.empty((rows, m), dtype=torch.int32).pin_memory()
@@ -242,7 +246,10 @@ def run_gpu(args):
             t = torch.tensor(total, dtype=torch.int64, device="cuda")
             gathered = [torch.zeros_like(t) for _ in range(world)]
             dist.all_gather(gathered, t)
-            total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
+            if weak:                                     # every rank counted everything: the copies must agree
+                assert all(g.tolist() == total for g in gathered), "ranks disagree (PAPER.md:99 duplicate-run check)"
+            else:
+                total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
         if rank == 0 and not args.profile_chunks:
             D, S = pb.pairings_reconstruct(kind, n, moduli, total)
             assert S == L20_IDENTIFIED and D == 2 * S, ("L(20) mismatch", D, S)
@@ -432,9 +439,10 @@ def run_gpu(args):
         cpu = cpu_baseline(kind, n) if not args.no_cpu else None
         line = dict(metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s", n_gpus=world,
                     steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=dev_ms / args.steps,
-                    higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
+                    higher_is_better=True, scaling=args.scaling, vs_baseline=None, dtype="int32", data="synthetic",
                     config=dict(workload=WORKLOAD,
-                                kind="langford", n=n, chunk_bits=C, n_moduli=m, parallelism="chunk ranges x%d" % world,
+                                kind="langford", n=n, chunk_bits=C, n_moduli=m, parallelism=("one full pass per GPU x%d, residue sums cross-checked" if weak else "disjoint chunk ranges x%d") % world,
+                                sm_count=torch.cuda.get_device_properties(local).multi_processor_count,
                                 l2="flushed between steps (256 MiB fill); the kernel reads no global memory",
                                 result_check="L(20) = 2,636,337,861,200 reconstructed every run (PAPER.md:380)",
                                 library=pb.pairings_build_info()),
@@ -460,6 +468,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
     ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 256 seeded S(24) runs to time")
+    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
+                    help="N > 1: weak = every rank a whole pass (cross-checked), strong = disjoint chunk ranges")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-pt", action="store_true", help="skip the approximate-counter (parallel tempering) measurement")
     ap.add_argument("--no-configs", action="store_true", help="skip the timing of the other BASELINE configs")
