@@ -248,6 +248,50 @@ PAIRINGS_HD uint32_t kconst(int zb, int bi, int r) {
 }
 
 // ------------------------------------------------------------------------------------------------
+// zero-step tables (row a4 for a whole 32-step block at once)
+// ------------------------------------------------------------------------------------------------
+// Within one inner block only the H inner bits move, so an even-distance sum P_d takes the values
+//     Q_d(S) = Q_d(0) + dQ_d(z(S), o),   z(S) = gray(S) the inner state, o = the signs of the (at most H)
+// outer positions that are partners of an inner position for this d.  dQ_d is a fixed function: pairs
+// (p, p+d) with p an inner index bit; the partner p+d is inner (p+d < H) or the outer index bit p+d.
+// For d >= H all H partners are outer and the function is the same for every d ("generic" shape); d = 2
+// and d = 4 have shapes of their own.  ztab[shape][Q_d(0) + ZR][o] is the 32-bit mask of the steps S at
+// which P_d vanishes; OR-ing the masks of the even slots gives every zero term of the block with ~5
+// instructions per slot and block instead of a 7-instruction test per step.
+constexpr int ZR = 24;                                   // rows for Q_d(0) in [-ZR, ZR]
+constexpr int ZSHAPES = 3;                               // 0: d >= H, 1: d = 2, 2: d = 4
+PAIRINGS_HD int zshape_of_d(int d) { return d >= H ? 0 : (d == 2 ? 1 : 2); }
+PAIRINGS_HD int zshape_d(int shape) { return shape == 0 ? H : (shape == 1 ? 2 : 4); }   // a representative distance
+struct ZeroTables { uint32_t t[ZSHAPES][2 * ZR + 1][32]; };
+PAIRINGS_HD int zcontrib(int d, int z, int o) {          // sum over inner p of x_p * x_{p+d}
+    int c = 0;
+    for (int p = 0; p < H; p++) {
+        const int xp = 1 - 2 * ((z >> p) & 1);
+        const int q = p + d;
+        // partner inside the inner bits, or pattern bit: outer index bit q, numbered from max(H, d)
+        const int xq = q < H ? 1 - 2 * ((z >> q) & 1) : 1 - 2 * ((o >> (q - (d >= H ? d : H))) & 1);
+        c += xp * xq;
+    }
+    return c;
+}
+PAIRINGS_HD ZeroTables make_zero_tables() {
+    ZeroTables T{};
+    for (int sh = 0; sh < ZSHAPES; sh++) {
+        const int d = zshape_d(sh);
+        for (int o = 0; o < 32; o++) {
+            const int c0 = zcontrib(d, 0, o);
+            for (int S = 0; S < BLK; S++) {                                  // Q(S) = q0 + dQ(S) = 0  <=>  q0 = -dQ(S)
+                const int dq = (zcontrib(d, gray_c(S), o) - c0) / 2;
+                T.t[sh][ZR - dq][o] |= 1u << S;
+            }
+        }
+    }
+    return T;
+}
+static_assert(H == 5 && BLK == 32, "the zero-step masks are 32-bit words indexed by 5 pattern bits");
+static __device__ constexpr ZeroTables g_ztab = make_zero_tables();
+
+// ------------------------------------------------------------------------------------------------
 // ring entry -> signed multi-word term -> accumulator
 // ------------------------------------------------------------------------------------------------
 template <int W>
@@ -341,6 +385,19 @@ __device__ __forceinline__ void sts_v2_pred(uint32_t addr, uint32_t a, uint32_t 
 __device__ __forceinline__ void sts_v1_pred(uint32_t addr, uint32_t a, uint32_t pred) {
     asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.shared.u32 [%0], %1;\n\t}"
                  :: "r"(addr), "r"(a), "r"(pred) : "memory");
+}
+// predicated on a CLEAR bit: store iff (word & bit) == 0 — the same test as the ballot's, so one predicate serves both
+__device__ __forceinline__ void sts_v4_clr(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t word, uint32_t bit) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %5, %6;\n\tsetp.eq.u32 p, t, 0;\n\t@p st.shared.v4.u32 [%0], {%1, %2, %3, %4};\n\t}"
+                 :: "r"(addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(word), "r"(bit) : "memory");
+}
+__device__ __forceinline__ void sts_v2_clr(uint32_t addr, uint32_t a, uint32_t b, uint32_t word, uint32_t bit) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %3, %4;\n\tsetp.eq.u32 p, t, 0;\n\t@p st.shared.v2.u32 [%0], {%1, %2};\n\t}"
+                 :: "r"(addr), "r"(a), "r"(b), "r"(word), "r"(bit) : "memory");
+}
+__device__ __forceinline__ void sts_v1_clr(uint32_t addr, uint32_t a, uint32_t word, uint32_t bit) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %2, %3;\n\tsetp.eq.u32 p, t, 0;\n\t@p st.shared.u32 [%0], %1;\n\t}"
+                 :: "r"(addr), "r"(a), "r"(word), "r"(bit) : "memory");
 }
 __device__ __forceinline__ void lds_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
@@ -476,13 +533,31 @@ struct Walker {
     uint32_t ring;            // shared-window byte address of this warp's ring (plane 0), RING_ALIGN-aligned
     uint32_t lane16;          // lane * 16
     uint32_t c80;             // 0x80808080 (KernelParams::c80)
+    uint32_t Vo;              // outer sign word: bit i = index bit H + i (set <-> x = -1)
+    uint32_t ZM;              // zero-step mask of the current block: bit S set <-> the term of step S has a zero factor
 
+    // Row a4 for the whole block: OR over the even-distance slots of the table masks (see ztab above).
+    __device__ __forceinline__ void zero_mask() {
+        uint32_t zm = 0;
+        static_for<0, L::n_even()>([&](auto sc) {
+            PAIRINGS_IC(s, sc);
+            constexpr int d = L::d_of_slot(s), sh = zshape_of_d(d);
+            static_assert(L::bound(s) <= ZR, "table rows");
+            const uint32_t u = __byte_perm(Q[s / 4], 0, 0x4440 + (s % 4));                 // biased byte Q + 128
+            uint32_t pat4;                                                                  // 4 * pattern (byte offset in the row)
+            if constexpr (d >= H + 2) pat4 = (Vo >> (d - H - 2)) & 0x7Cu;
+            else if constexpr (d >= H) pat4 = (Vo << (H + 2 - d)) & 0x7Cu;
+            else pat4 = (Vo << 2) & (((1u << d) - 1u) << 2);
+            const unsigned char* row = reinterpret_cast<const unsigned char*>(&g_ztab.t[sh][0][0]) + (ZR - 128) * 128;
+            zm |= *reinterpret_cast<const uint32_t*>(row + (size_t)u * 128u + pat4);
+        });
+        ZM = zm;
+    }
+
+    template <int S>
     __device__ __forceinline__ void push_if_nonzero(uint32_t sgnword) {
-        uint32_t z = 0;
-#pragma unroll
-        for (int r = 0; r < NT; r++) z |= Q[r] & ~(Q[r] - 0x01010101u);
-        const uint32_t nonzero = ((z & 0x80808080u) == 0) ? 1u : 0u;
-        const uint32_t bal = __ballot_sync(0xffffffffu, nonzero != 0);
+        constexpr uint32_t bit = 1u << S;
+        const uint32_t bal = __ballot_sync(0xffffffffu, (ZM & bit) == 0);
         // slot = (tail + rank among the warp's non-zero lanes) mod QCAP; ring is aligned, so "|" adds the offset
         const uint32_t addr = ((tail16 + 16u * (uint32_t)__popc(bal & ltmask)) & (uint32_t)(PLANE_BYTES - 16)) | ring;
         // entry words: Q[0..NR), sign; plane p holds words 4p..4p+3 (predicated vector stores, no branch)
@@ -492,9 +567,9 @@ struct Walker {
         static_for<0, L::PLANES>([&](auto pc) {
             PAIRINGS_IC(pl, pc);
             constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
-            if constexpr (words >= 3) sts_v4_pred(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], nonzero);
-            else if constexpr (words == 2) sts_v2_pred(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], nonzero);
-            else sts_v1_pred(addr + pl * PLANE_BYTES, e[4 * pl], nonzero);
+            if constexpr (words >= 3) sts_v4_clr(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
+            else if constexpr (words == 2) sts_v2_clr(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
+            else sts_v1_clr(addr + pl * PLANE_BYTES, e[4 * pl], ZM, bit);
         });
         tail16 += 16u * (uint32_t)__popc(bal);
     }
@@ -526,7 +601,7 @@ struct Walker {
     __device__ __forceinline__ void quad() {
         static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
             PAIRINGS_IC(S, sc);
-            push_if_nonzero((S & 1) ? sgn_odd : sgn_even);
+            push_if_nonzero<S>((S & 1) ? sgn_odd : sgn_even);
             if constexpr (S + 1 < BLK) inner_flip<zbits(S), ctz_c(S + 1)>();
         });
     }
@@ -570,6 +645,7 @@ struct Walker {
             }
         });
         if (b & 1) O ^= 1u << (b >> 1); else E ^= 1u << (b >> 1);
+        Vo ^= 1u << (b - H);
     }
 
     template <int b>
@@ -604,6 +680,7 @@ struct Walker {
             o |= (uint32_t)((V >> (2 * i + 1)) & 1ULL) << i;
         }
         E = e; O = o;
+        Vo = (uint32_t)(V >> H);
         static_for<0, H>([&](auto bc) { PAIRINGS_IC(bi, bc); LeftVec<KIND, NN, bi, true>::eval(E, O, C[bi]); });
         const int s0 = (__popcll(V) & 1) ? -1 : 1;
         sgn_even = (uint32_t)s0; sgn_odd = (uint32_t)(-s0);
@@ -657,6 +734,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
         // One inner block = BLK unrolled steps from inner state 0, a drain check every QUAD steps.
 #pragma unroll 1
         for (uint32_t u = 0; u < nblk; u++) {
+            wk.zero_mask();
             static_for<0, BLK / QUAD>([&](auto qc) {
                 PAIRINGS_IC(QI, qc);
                 wk.template quad<QI>();
