@@ -262,7 +262,7 @@ constexpr int ZR = 24;                                   // rows for Q_d(0) in [
 constexpr int ZSHAPES = 3;                               // 0: d >= H, 1: d = 2, 2: d = 4
 PAIRINGS_HD int zshape_of_d(int d) { return d >= H ? 0 : (d == 2 ? 1 : 2); }
 PAIRINGS_HD int zshape_d(int shape) { return shape == 0 ? H : (shape == 1 ? 2 : 4); }   // a representative distance
-struct ZeroTables { uint32_t t[ZSHAPES][2 * ZR + 1][32]; };
+struct alignas(128) ZeroTables { uint32_t t[ZSHAPES][2 * ZR + 1][32]; };
 PAIRINGS_HD int zcontrib(int d, int z, int o) {          // sum over inner p of x_p * x_{p+d}
     int c = 0;
     for (int p = 0; p < H; p++) {
@@ -548,8 +548,15 @@ struct Walker {
             if constexpr (d >= H + 2) pat4 = (Vo >> (d - H - 2)) & 0x7Cu;
             else if constexpr (d >= H) pat4 = (Vo << (H + 2 - d)) & 0x7Cu;
             else pat4 = (Vo << 2) & (((1u << d) - 1u) << 2);
-            const unsigned char* row = reinterpret_cast<const unsigned char*>(&g_ztab.t[sh][0][0]) + (ZR - 128) * 128;
-            zm |= *reinterpret_cast<const uint32_t*>(row + (size_t)u * 128u + pat4);
+            // address = table(shape) + (u - 128 + ZR) * 128 + pat4: the tables are 128-byte aligned, so pat4 is OR-ed
+            // into the low word of the (biased) base and ONE wide multiply-add forms the 64-bit address
+            const uint64_t base = (uint64_t)(uintptr_t)(&g_ztab.t[sh][0][0]) + (uint64_t)(int64_t)((ZR - 128) * 128);
+            uint64_t addr;
+            asm("{\n\t.reg .b32 lo, hi;\n\t.reg .b64 bp;\n\tmov.b64 {lo, hi}, %2;\n\tor.b32 lo, lo, %3;\n\tmov.b64 bp, {lo, hi};\n\t"
+                "mad.wide.u32 %0, %1, 128, bp;\n\t}" : "=l"(addr) : "r"(u), "l"(base), "r"(pat4));
+            uint32_t mask;
+            asm("ld.global.nc.u32 %0, [%1];" : "=r"(mask) : "l"(addr));
+            zm |= mask;
         });
         ZM = zm;
     }
