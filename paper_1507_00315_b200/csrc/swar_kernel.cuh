@@ -696,7 +696,7 @@ struct Walker {
 
 template <int KIND, int NN>
 #ifndef PAIRINGS_SWAR_MINB
-#define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM (the ring limits it to 3 anyway): at most 85 registers
+#define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM (the ring limits it to 3 anyway): at most 85 registers; measured faster than 2 blocks without spills at n = 24
 #endif
 __global__ void __launch_bounds__(256, PAIRINGS_SWAR_MINB)
 swar_kernel(const __grid_constant__ KernelParams kp) {
