@@ -6,8 +6,8 @@
 //  * pair-sums live byte-packed, four per 32-bit register ("slots"): slot value = Q_k + 128 with
 //    Q_k = P_k/2 for even d_k (P_k = N-d_k mod 2, so these are the only sums that can vanish) and
 //    Q_k = P_k for odd d_k.  The factor 2^{#even} is restored once per thread at the end.
-//    Even-d slots come first, so the zero test (row a4) looks at NT = ceil(#even/4) registers:
-//    a byte is 0x80 iff  bit7(v) & ~bit7(v - 0x01010101).
+//    Even-d slots come first.  The zero test (row a4) is done for a whole inner block at once from
+//    compile-time tables (see "zero-step tables" below): one 32-bit mask of the zero steps per block.
 //  * the low H = 5 index bits are walked by ONE fully unrolled 32-step Gray block that always starts
 //    in inner state 0.  For every inner position the packed vector C[b] of its neighbours that lie
 //    OUTSIDE the inner bits is kept in registers; neighbours inside the inner bits are known at
@@ -449,7 +449,7 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
             gp[g] *= v;                                                           // exact: |group| < 2^31
         }
     });
-    if constexpr (G <= 3) {
+    if constexpr (G <= 4) {
         // signed multi-word product T = gp[0] * gp[1] * ... (two's complement, top word signed).  A k-word T
         // times a signed 32-bit m: the k-1 low (unsigned) words are multiplied by m read as unsigned, i.e.
         // by m + 2^32 [m < 0], and that excess — the low words shifted up one word — is subtracted again.
