@@ -158,7 +158,11 @@ struct Lay {
     static constexpr int W = (plan.bits + 33 + 31) / 32;
     static_assert(G >= 1, "no grouping found");
     static_assert(W >= G && W <= 8, "accumulator must hold the multi-word product");
-    static constexpr int EW = NR + 1;                   // ring entry words (packed sums + sign)
+    // The sign of a term, prod_i x_i = (-1)^{#(x_i = -1)}, is not stored: for d = n the pairs (i, i+n) cover every
+    // position exactly once, so #(x_i != x_{i+n}) = (n - P_n)/2 has the parity of #(x_i = -1).
+    static constexpr int SIGN_SLOT = slot_of_d(NN);     // exists for both kinds (Skolem k = n, Langford k = n-1)
+    static_assert(SIGN_SLOT >= 0, "distance n");
+    static constexpr int EW = NR;                       // ring entry words (the packed sums)
     static constexpr int PLANES = (EW + 3) / 4;         // 16-byte planes per entry
     static constexpr uint32_t PAD = 0x40;               // value of unused slots (never reads as zero)
 };
@@ -430,7 +434,15 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
     int gp[G];
 #pragma unroll
     for (int g = 0; g < G; g++) gp[g] = 1;
-    gp[0] = (int)e[NR];                                                           // sign of the term
+    // sign of the term from the slot of distance n (biased byte u): n even: Q = P/2 = n/2 - pc, pc odd <=> (u ^ n/2) odd;
+    // n odd: Q = P = n - 2 pc, pc odd <=> bit 1 of (u - n) set.  (Subtracting inside byte i never borrows from below.)
+    {
+        constexpr int r = L::SIGN_SLOT / 4, i = L::SIGN_SLOT % 4;
+        bool negative;
+        if constexpr (NN % 2 == 0) negative = (((e[r] >> (8 * i)) ^ (uint32_t)(NN / 2)) & 1u) != 0;
+        else negative = (((e[r] - ((uint32_t)NN << (8 * i))) >> (8 * i + 1)) & 1u) != 0;
+        gp[0] = negative ? -1 : 1;
+    }
     static_for<0, L::NF_MAX>([&](auto fc) {
         PAIRINGS_IC(f, fc);
         if constexpr (f < L::plan.nf) {
@@ -528,7 +540,6 @@ struct Walker {
     uint32_t E, O;            // de-interleaved sign word: E bit i = index bit 2i, O bit i = index bit 2i+1
     uint32_t acc[W];
     uint32_t tail16, head16;  // warp-uniform ring counters (monotone), in units of 1/16 entry (= byte offsets)
-    uint32_t sgn_even, sgn_odd;   // sign word pushed at even / odd inner steps (+1 / -1 as int)
     uint32_t ltmask;
     uint32_t ring;            // shared-window byte address of this warp's ring (plane 0), RING_ALIGN-aligned
     uint32_t lane16;          // lane * 16
@@ -562,7 +573,7 @@ struct Walker {
     }
 
     template <int S>
-    __device__ __forceinline__ void push_if_nonzero(uint32_t sgnword) {
+    __device__ __forceinline__ void push_if_nonzero() {
         constexpr uint32_t bit = 1u << S;
         const uint32_t bal = __ballot_sync(0xffffffffu, (ZM & bit) == 0);
         // slot = (tail + rank among the warp's non-zero lanes) mod QCAP; ring is aligned, so "|" adds the offset
@@ -570,7 +581,7 @@ struct Walker {
         // entry words: Q[0..NR), sign; plane p holds words 4p..4p+3 (predicated vector stores, no branch)
         uint32_t e[4 * L::PLANES];
 #pragma unroll
-        for (int i = 0; i < 4 * L::PLANES; i++) e[i] = (i < NR) ? Q[i] : sgnword;
+        for (int i = 0; i < 4 * L::PLANES; i++) e[i] = Q[i < NR ? i : 0];
         static_for<0, L::PLANES>([&](auto pc) {
             PAIRINGS_IC(pl, pc);
             constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
@@ -608,7 +619,7 @@ struct Walker {
     __device__ __forceinline__ void quad() {
         static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
             PAIRINGS_IC(S, sc);
-            push_if_nonzero<S>((S & 1) ? sgn_odd : sgn_even);
+            push_if_nonzero<S>();
             if constexpr (S + 1 < BLK) inner_flip<zbits(S), ctz_c(S + 1)>();
         });
     }
@@ -626,12 +637,10 @@ struct Walker {
     }
 
     // Between two blocks: the inner walk ended in state 1 << (H-1); flip that bit back so that every
-    // block runs the same compile-time sequence from inner state 0, then flip outer bit `bit`.  The
-    // two flips keep the sign of the term, so the signs pushed at even / odd steps swap.
+    // block runs the same compile-time sequence from inner state 0, then flip outer bit `bit`.
     __device__ __forceinline__ void block_end(int bit) {
         inner_flip<(1 << (H - 1)), H - 1>();
         outer_flip_dispatch<H>(bit);
-        const uint32_t t = sgn_even; sgn_even = sgn_odd; sgn_odd = t;
     }
 
     // flip of index bit b >= H (between two inner blocks)
@@ -689,8 +698,6 @@ struct Walker {
         E = e; O = o;
         Vo = (uint32_t)(V >> H);
         static_for<0, H>([&](auto bc) { PAIRINGS_IC(bi, bc); LeftVec<KIND, NN, bi, true>::eval(E, O, C[bi]); });
-        const int s0 = (__popcll(V) & 1) ? -1 : 1;
-        sgn_even = (uint32_t)s0; sgn_odd = (uint32_t)(-s0);
     }
 };
 
