@@ -277,8 +277,9 @@ def default_chunk_bits(n: int) -> int:
 
 
 def default_chunks_per_call(n: int, chunk_bits: int) -> int:
-    """About 2^38 sign vectors per kernel call (a fraction of a second): few launches, journal lines, D2H copies."""
-    return 1 << max(0, min(chunk_bits, 38 - (2 * n - 1 - chunk_bits)))
+    """About 2^41 sign vectors per kernel call (a few seconds): few launches, journal lines, D2H copies, and a
+    last partly filled wave of blocks that is short against the call."""
+    return 1 << max(0, min(chunk_bits, 41 - (2 * n - 1 - chunk_bits)))
 
 
 def count(kind: int, n: int, chunk_bits: Optional[int] = None, n_moduli: Optional[int] = None,
