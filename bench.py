@@ -42,8 +42,9 @@ WL = dict(kind=1, n=20, chunk_bits=16, n_moduli=7)
 L20_IDENTIFIED = 2636337861200          # L(20), PAPER.md:380 (Table 8)
 WORKLOAD = "L(20): Langford n=20, 2^39 sign vectors (x_1=+1), 2^16 prefix chunks, 6 CRT primes + 1 check prime, full count per step"
 # secondary point of the metric (configs[4]): Skolem n = 24, 2^20 chunks, 8 primes + 1 check prime,
-# a fixed seeded 1/64 subset of chunks (256 runs of 64 contiguous chunks)
-WL24 = dict(kind=0, n=24, chunk_bits=20, n_moduli=9, runs=256, run_len=64)
+# a fixed seeded 1/64 subset of chunks (16 runs of 1024 contiguous chunks: launches long enough that the last,
+# partly filled wave of blocks does not dominate)
+WL24 = dict(kind=0, n=24, chunk_bits=20, n_moduli=9, runs=16, run_len=1024)
 # BASELINE.json configs[0..3] other than the workload: (kind, n, chunk_bits, moduli incl. check, back-to-back
 # launches timed, printed count: PAPER.md Table 8 :376,:378 / Table 7 :351,:352,:354)
 OTHER_CONFIGS = [(1, 12, 6, 4, 100, 108144), (0, 13, 8, 4, 100, 1520280), (1, 16, 10, 6, 20, 326721800),
@@ -467,7 +468,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
-    ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 256 seeded S(24) runs to time")
+    ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 16 seeded S(24) runs (1024 chunks each) to time")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
                     help="N > 1: weak = every rank a whole pass (cross-checked), strong = disjoint chunk ranges")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
