@@ -271,3 +271,17 @@ def test_lemma24_x2_half_is_half_the_sum_or_cancels(kind, n):
         assert t0 == t1 and 2 * t0 == oracle.brute_count(kind, n) << (2 * n - 1)
     else:
         assert t0 == -t1 and oracle.brute_count(kind, n) == 0
+
+
+@pytest.mark.parametrize("kind,n", [(S, 4), (S, 5), (S, 8), (L, 7), (L, 8), (S, 13), (L, 20), (S, 21), (S, 24)])
+def test_sign_of_a_term_is_the_parity_of_the_distance_n_sum(kind, n):
+    # The pairs (i, i+n), i = 1..n, cover every position exactly once, so #(x_i != x_{i+n}) = (n - P_n)/2 has the
+    # parity of #(x_i = -1) and prod_i x_i = (-1)^{(n - P_n)/2}.  (The SWAR kernel does not store the sign of a
+    # queued term, it reads it off the distance-n sum; both kinds have a pair of distance n.)
+    rng = random.Random(1000 * kind + n)
+    assert n in [(k if kind == S else k + 1) for k in range(1, n + 1)]
+    for _ in range(200):
+        x = [rng.choice((1, -1)) for _ in range(2 * n)]
+        Pn = sum(x[i] * x[i + n] for i in range(n))
+        assert (n - Pn) % 2 == 0
+        assert math.prod(x) == (-1) ** ((n - Pn) // 2)
