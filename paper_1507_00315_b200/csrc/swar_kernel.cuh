@@ -262,7 +262,7 @@ PAIRINGS_HD uint32_t kconst(int zb, int bi, int r) {
 // and d = 4 have shapes of their own.  ztab[shape][Q_d(0) + ZR][o] is the 32-bit mask of the steps S at
 // which P_d vanishes; OR-ing the masks of the even slots gives every zero term of the block with ~5
 // instructions per slot and block instead of a 7-instruction test per step.
-constexpr int ZR = 24;                                   // rows for Q_d(0) in [-ZR, ZR]
+constexpr int ZR = 31;                                   // rows for Q_d(0) in [-ZR, ZR]  (n <= 32: |Q| <= 31)
 constexpr int ZSHAPES = 3;                               // 0: d >= H, 1: d = 2, 2: d = 4
 PAIRINGS_HD int zshape_of_d(int d) { return d >= H ? 0 : (d == 2 ? 1 : 2); }
 PAIRINGS_HD int zshape_d(int shape) { return shape == 0 ? H : (shape == 1 ? 2 : 4); }   // a representative distance

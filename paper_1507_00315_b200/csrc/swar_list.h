@@ -5,6 +5,6 @@
 #define PAIRINGS_SWAR_H 5
 #ifndef PAIRINGS_SWAR_LIST
 #define PAIRINGS_SWAR_LIST(X) \
-    X(0, 8) X(0, 12) X(0, 13) X(0, 16) X(0, 20) X(0, 21) X(0, 24) \
-    X(1, 7) X(1, 8) X(1, 11) X(1, 12) X(1, 16) X(1, 20) X(1, 24)
+    X(0, 8) X(0, 9) X(0, 12) X(0, 13) X(0, 16) X(0, 17) X(0, 20) X(0, 21) X(0, 24) X(0, 25) \
+    X(1, 7) X(1, 8) X(1, 11) X(1, 12) X(1, 15) X(1, 16) X(1, 19) X(1, 20) X(1, 23) X(1, 24) X(1, 27)
 #endif

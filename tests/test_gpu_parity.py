@@ -275,3 +275,27 @@ def test_duplicate_run_mode_and_tight_moduli(kind, n, C, paper_counts):
     D, Sid = pb.pairings_reconstruct(kind, n, moduli, total)
     assert Sid == paper_counts[(kind, n)] and D == 2 * Sid
     assert pb.count(kind, n, duplicate=True, tight_moduli=True) == (D, Sid)
+
+
+# ---- the remaining exact values of Tables 7/8 the SWAR kernel is compiled for
+@pytest.mark.parametrize("kind,n,C,count,pieces", [(S, 9, 4, 16, 1), (L, 15, 12, 8, 1), (S, 17, 16, 8, 1), (L, 19, 20, 8, 1),
+                                                   (L, 23, 22, 3, 16), (S, 25, 26, 3, 16), (L, 27, 30, 3, 16)])
+def test_more_instances_sampled_chunks_match_oracle(kind, n, C, count, pieces):
+    assert pb.pairings_has_swar(kind, n)
+    moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)
+    chunks = seeds.sample_chunks(C, count, salt=300 + n)
+    want = oracle_rows(kind, n, C, chunks, moduli, threads=16, pieces=pieces)
+    for c, w in zip(chunks, want):
+        b = min(c & ~31, (1 << C) - 32) if C >= 5 else 0
+        e = min(b + 32, 1 << C)
+        rows, nz = gpu_rows(kind, n, C, b, e, moduli, pb.LaunchOpts(variant=pb.VARIANT_SWAR), count_nonzero=False), None
+        assert rows[c - b] == w[2], (kind, n, c)
+        assert pb.pairings_crt_signed(moduli, rows[c - b]) == w[0]
+
+
+@pytest.mark.parametrize("kind,n", [(S, 9), (L, 15), (S, 17), (L, 19)])
+def test_more_paper_totals(kind, n, paper_counts):
+    # PAPER.md:349 (S(9)), :352 (S(17)), :377 (L(15)), :379 (L(19))
+    full = pb.count(kind, n)
+    assert full[1] == paper_counts[(kind, n)] and full[0] == 2 * full[1]
+    assert pb.count(kind, n, lemma24=True, duplicate=True) == full
