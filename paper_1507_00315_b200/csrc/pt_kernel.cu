@@ -16,7 +16,8 @@
 //   occ[slot][b]   balls in bin b                                                M x (2n+1) bytes
 //   lev[j] = slot holding level j's configuration, E[j] its energy               2 M bytes
 // An exchange swaps lev / E entries, not configurations.  The energy change of a move is counted
-// incrementally: bins that become empty minus bins that become occupied.
+// incrementally from the occupancy of the four affected bins: bins that become empty minus bins that
+// become occupied.
 #include "pairings.h"
 #include "internal.h"
 
@@ -88,34 +89,46 @@ __global__ void __launch_bounds__(PT_THREADS) pt_kernel(const PtParams p) {
             // ---- step 1: ratio samples
             const bool counted = t >= p.burn_in;
             if (counted) for (int j = 0; j < M; j++) atomicAdd(&shist[j * (N + 1) + ST(EN + j)], 1u);
-            // ---- step 2: one move per level
-            for (int j = 0; j < M; j++) {
-                const int slot = ST(LEV + j);
+            // ---- step 2: one move per level.  A move is evaluated from loads only (the four affected bins and
+            // the old position), so the moves of two levels — different configurations — are evaluated together
+            // and their dependent load chains overlap; shared memory is written only when a move is accepted.
+            struct Move { int slot, k, d, a0, a1, dE, j; };
+            auto evaluate = [&](int j) -> Move {
+                Move m; m.j = j;
+                m.slot = ST(LEV + j);
                 const uint64_t w = pt_draw(seed, (base + j) * S + 0);
-                const int k = 1 + (int)(((w & 0xFFFFFFFFULL) * (uint64_t)n) >> 32);
-                const int d = dist(kind, k);
-                const int a1 = 1 + (int)(((w >> 32) * (uint64_t)(N - d)) >> 32);
-                const int a0 = ST(POS + slot * n + (k - 1));
-                const int ob = OCC + slot * (N + 1);
-                int dE = 0;
-                unsigned char c;
-                c = ST(ob + a0) - 1; ST(ob + a0) = c; dE += (c == 0);
-                c = ST(ob + a0 + d) - 1; ST(ob + a0 + d) = c; dE += (c == 0);
-                c = ST(ob + a1) + 1; ST(ob + a1) = c; dE -= (c == 1);
-                c = ST(ob + a1 + d) + 1; ST(ob + a1 + d) = c; dE -= (c == 1);
-                bool accept = dE <= 0;
+                m.k = 1 + (int)(((w & 0xFFFFFFFFULL) * (uint64_t)n) >> 32);
+                m.d = dist(kind, m.k);
+                m.a1 = 1 + (int)(((w >> 32) * (uint64_t)(N - m.d)) >> 32);
+                m.a0 = ST(POS + m.slot * n + (m.k - 1));
+                const int ob = OCC + m.slot * (N + 1);
+                const int c0 = ST(ob + m.a0), c1 = ST(ob + m.a0 + m.d), c2 = ST(ob + m.a1), c3 = ST(ob + m.a1 + m.d);
+                // bins that become empty when the pair leaves (a0 != a0+d), minus bins that are empty after that
+                // and become occupied when it lands (a1 != a1+d); a bin left and re-entered counts in both
+                const int e2 = (m.a1 == m.a0) + (m.a1 == m.a0 + m.d), e3 = (m.a1 + m.d == m.a0) + (m.a1 + m.d == m.a0 + m.d);
+                m.dE = (c0 == 1) + (c1 == 1) - (c2 - e2 == 0) - (c3 - e3 == 0);
+                return m;
+            };
+            auto commit = [&](const Move& m) {
+                bool accept = m.dE <= 0;
                 if (!accept) {
-                    const uint64_t u = pt_draw(seed, (base + j) * S + 1) >> 32;
-                    accept = u < p.move_thr[j * 2 + (dE - 1)];
+                    const uint64_t u = pt_draw(seed, (base + m.j) * S + 1) >> 32;
+                    accept = u < p.move_thr[m.j * 2 + (m.dE - 1)];
                 }
                 if (accept) {
-                    ST(POS + slot * n + (k - 1)) = (unsigned char)a1;
-                    ST(EN + j) = (unsigned char)((int)ST(EN + j) + dE);
-                    if (counted) atomicAdd(&smoves[j], 1u);
-                } else {
-                    ST(ob + a1) -= 1; ST(ob + a1 + d) -= 1; ST(ob + a0) += 1; ST(ob + a0 + d) += 1;
+                    const int ob = OCC + m.slot * (N + 1);
+                    ST(ob + m.a0) -= 1; ST(ob + m.a0 + m.d) -= 1; ST(ob + m.a1) += 1; ST(ob + m.a1 + m.d) += 1;
+                    ST(POS + m.slot * n + (m.k - 1)) = (unsigned char)m.a1;
+                    ST(EN + m.j) = (unsigned char)((int)ST(EN + m.j) + m.dE);
+                    if (counted) atomicAdd(&smoves[m.j], 1u);
                 }
+            };
+            int j2 = 0;
+            for (; j2 + 1 < M; j2 += 2) {
+                const Move ma = evaluate(j2), mb = evaluate(j2 + 1);
+                commit(ma); commit(mb);
             }
+            if (j2 < M) commit(evaluate(j2));
             // ---- step 3: exchanges j, j+1 in sequence
             for (int j = 0; j + 1 < M; j++) {
                 const int e0 = ST(EN + j), e1 = ST(EN + j + 1), dE = e0 - e1;
