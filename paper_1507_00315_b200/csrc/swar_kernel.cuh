@@ -22,7 +22,7 @@
 //    the sign word with a multiply-spread (4 bits -> 4 bytes), and patches one byte of each C[b].
 //    Because g <= n-2, every left neighbour of a walked position exists: no boundary guards at all.
 //  * non-zero terms are compacted (row a4's divergence problem): ballot + popc prefix push the packed
-//    registers + sign into a per-warp shared-memory ring; whenever 32 entries are queued all lanes
+//    registers into a per-warp shared-memory ring (the sign of the term is read off the distance-n sum); whenever 32 entries are queued all lanes
 //    multiply one entry each (any lane may process any term of its warp: the sum is commutative and
 //    a warp never spans two chunks).
 //  * row a5: the product is formed from dp4a "pair factors" (two sums per LOP3 + IDP.4A), G exact
@@ -87,7 +87,6 @@ struct Lay {
     PAIRINGS_HD static int cnt(int s) { return N - d_of_slot(s); }                     // number of summands of P
     PAIRINGS_HD static int bound(int s) { return d_of_slot(s) % 2 == 0 ? cnt(s) / 2 : cnt(s); }   // |Q| <= bound
     static constexpr int NR = (NN + 3) / 4;            // packed registers
-    static constexpr int NT = (n_even() + 3) / 4;      // registers that need the zero test
     // ---- product plan (row a5).  The n factors are multiplied as "pair factors": byte i of register
     // 2p times byte i of register 2p+1 in ONE dp4a (the second operand masked to that byte), bytes
     // (0,1) and (2,3) of an unpaired last register likewise; a slot without a partner is a single
@@ -378,18 +377,6 @@ __device__ __forceinline__ void acc_add(uint32_t (&acc)[W], const uint32_t (&x)[
     }
 }
 
-__device__ __forceinline__ void sts_v4_pred(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t pred) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %5, 0;\n\t@p st.shared.v4.u32 [%0], {%1, %2, %3, %4};\n\t}"
-                 :: "r"(addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(pred) : "memory");
-}
-__device__ __forceinline__ void sts_v2_pred(uint32_t addr, uint32_t a, uint32_t b, uint32_t pred) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %3, 0;\n\t@p st.shared.v2.u32 [%0], {%1, %2};\n\t}"
-                 :: "r"(addr), "r"(a), "r"(b), "r"(pred) : "memory");
-}
-__device__ __forceinline__ void sts_v1_pred(uint32_t addr, uint32_t a, uint32_t pred) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.u32 p, %2, 0;\n\t@p st.shared.u32 [%0], %1;\n\t}"
-                 :: "r"(addr), "r"(a), "r"(pred) : "memory");
-}
 // predicated on a CLEAR bit: store iff (word & bit) == 0 — the same test as the ballot's, so one predicate serves both
 __device__ __forceinline__ void sts_v4_clr(uint32_t addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t word, uint32_t bit) {
     asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %5, %6;\n\tsetp.eq.u32 p, t, 0;\n\t@p st.shared.v4.u32 [%0], {%1, %2, %3, %4};\n\t}"
@@ -533,7 +520,7 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
 template <int KIND, int NN>
 struct Walker {
     using L = Lay<KIND, NN>;
-    static constexpr int NR = L::NR, NT = L::NT, W = L::W, EW = L::EW;
+    static constexpr int NR = L::NR, W = L::W, EW = L::EW;
 
     uint32_t Q[NR];
     uint32_t C[H][NR];
