@@ -203,6 +203,9 @@ def run_gpu(args):
     import paper_1507_00315_b200 as pb
     from paper_1507_00315_b200 import seeds
 
+    from paper_1507_00315_b200 import build as pbuild
+    if not os.path.exists(pb.library_path()):
+        pbuild.build()                         # fresh checkout: build in-tree (nvcc, sm_100a)
     pb.lib()                                   # fails loudly if the CUDA library is missing
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))

@@ -14,6 +14,14 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
+@pytest.fixture(scope="session", autouse=True)
+def built_library():
+    """The CUDA library is built in-tree (nvcc, sm_100a) if it is missing or older than its sources; the tests never
+    fall back to anything else."""
+    from paper_1507_00315_b200 import build as pbuild
+    return pbuild.build()
+
+
 def read_golden(name):
     rows = []
     with open(os.path.join(GOLDEN, name)) as f:
