@@ -253,6 +253,16 @@ int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
                     uint64_t replica_begin, uint64_t replica_end, uint64_t iterations, uint64_t burn_in, uint64_t seed,
                     uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream);
 
+/* Ladder choice (exchange acceptance "no smaller than one half", as few levels as that allows).
+ * Builds betas_out[0] = 0 < betas_out[1] < ... level by level: a pilot run (pilot_replicas x pilot_iterations, half
+ * of them burn-in) of the ladder so far gives the energy distribution of its last level, and the next beta is the
+ * one whose predicted exchange acceptance with it (by reweighting) equals target_exchange (at most a doubling of
+ * beta per level); stops when the last level is at E = 0 with probability >= 0.98 or beta >= 32.  Deterministic in (kind, n, target, pilot sizes, seed).  Synchronises
+ * the stream.  Returns the number of levels (<= cap_levels, <= PAIRINGS_PT_MAX_LEVELS) or a negative code
+ * (PAIRINGS_ERANGE: cap reached first).  betas_out: HOST, cap_levels doubles. */
+int pairings_pt_ladder(int kind, int n, double target_exchange, uint64_t pilot_replicas, uint64_t pilot_iterations,
+                       uint64_t seed, double* betas_out, int cap_levels, void* stream);
+
 /* Host: Ratio(j)/iterations of Algorithm 2 from the histogram (HOST, n_levels x (2n+1)),
  *     ratios_out[j] = sum_E hist[j][E] exp(-(beta(j+1) - beta(j)) E) / sum_E hist[j][E]     (last level: [E = 0]),
  * and *log_distinct_out = log( Z(0) prod_j ratios[j] ), the natural logarithm of the estimated number of

@@ -12,6 +12,6 @@ from .api import (  # noqa: F401
     pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_lemma24, RUN_LEMMA24, RUN_DUPLICATE,
     default_chunk_bits, default_chunks_per_call,
     pairings_reconstruct, pairings_crt_signed, pairings_strerror, pairings_build_info,
-    pairings_issue_probe, pairings_pt_run, pairings_pt_estimate,
-    count,
+    pairings_issue_probe, pairings_pt_run, pairings_pt_estimate, pairings_pt_ladder,
+    count, approx_count,
 )

@@ -30,6 +30,10 @@ def main(argv=None) -> int:
                     help="PAPER.md:99: evaluate every chunk range twice (other launch geometry), third run on mismatch")
     ap.add_argument("--tight-moduli", action="store_true",
                     help="size the prime set from 2^(2n-1) prod(2n-d_k) instead of (2n)^n 2^(2n)")
+    ap.add_argument("--approx", action="store_true",
+                    help="approximate count by parallel tempering (PAPER.md section 3) instead of the exact count")
+    ap.add_argument("--replicas", type=int, default=1 << 12)
+    ap.add_argument("--iterations", type=int, default=None, help="per replica (default 2^16, 2^21 for n >= 20, 2^23 for n >= 24)")
     ap.add_argument("--journal", default=None)
     ap.add_argument("--max-calls", type=int, default=0)
     ap.add_argument("--json", action="store_true")
@@ -37,6 +41,17 @@ def main(argv=None) -> int:
 
     kind = api.SKOLEM if a.kind.upper() == "S" else api.LANGFORD
     n = a.n
+    if a.approx:
+        its = a.iterations if a.iterations is not None else (1 << 16 if n < 20 else (1 << 21 if n < 24 else 1 << 23))
+        t0 = time.perf_counter()
+        r = api.approx_count(kind, n, a.replicas, its)
+        r["seconds"] = time.perf_counter() - t0
+        if a.json:
+            print(json.dumps(r))
+        else:
+            print("%s(%d) ~ %.6g (reflections identified; %d levels, %.3g samples per level, %.2f s)" %
+                  (a.kind.upper(), n, r["identified"], len(r["betas"]), r["samples"], r["seconds"]))
+        return 0
     m = a.moduli if a.moduli is not None else \
         (api.pairings_min_moduli(kind, n) if a.tight_moduli else api.pairings_bound_moduli(kind, n)) + 1
     moduli = api.pairings_default_moduli(m)

@@ -65,6 +65,7 @@ def lib():
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
         "pairings_pt_run": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64, u64, u64, u64, u64, vp, vp, vp, vp]),
+        "pairings_pt_ladder": (i, [i, i, ctypes.c_double, u64, u64, u64, ctypes.POINTER(ctypes.c_double), i, vp]),
         "pairings_pt_estimate": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64p, ctypes.POINTER(ctypes.c_double),
                                      ctypes.POINTER(ctypes.c_double)]),
         "pairings_issue_probe": (i, [i, i, i, i, vp, vp, u64p]),
@@ -260,6 +261,15 @@ def pairings_pt_run(kind, n, betas, replica_begin, replica_end, iterations, burn
                                  ctypes.c_void_p(swaps_dev_ptr), ctypes.c_void_p(stream)), "pairings_pt_run")
 
 
+def pairings_pt_ladder(kind, n, target_exchange=0.55, pilot_replicas=256, pilot_iterations=1 << 14, seed=1,
+                       cap_levels=32, stream: int = 0):
+    """Inverse-temperature ladder with the given predicted exchange acceptance.  Returns the betas."""
+    out = (ctypes.c_double * cap_levels)()
+    m = _check(lib().pairings_pt_ladder(kind, n, target_exchange, pilot_replicas, pilot_iterations, seed, out,
+                                        cap_levels, ctypes.c_void_p(stream)), "pairings_pt_ladder")
+    return [float(out[j]) for j in range(m)]
+
+
 def pairings_pt_estimate(kind, n, betas, hist):
     """hist: levels x (2n+1) counts.  Returns (ratios per level, log of the estimated reflections-distinct count)."""
     M = len(betas)
@@ -269,6 +279,34 @@ def pairings_pt_estimate(kind, n, betas, hist):
     lz = ctypes.c_double(0.0)
     _check(lib().pairings_pt_estimate(kind, n, b, M, flat, r, ctypes.byref(lz)), "pairings_pt_estimate")
     return [float(v) for v in r], float(lz.value)
+
+
+def approx_count(kind: int, n: int, replicas: int = 1 << 12, iterations: int = 1 << 16, burn_in: Optional[int] = None,
+                 seed: int = 150700315, betas=None, target_exchange: float = 0.55, device_alloc=None):
+    """Convenience: the approximate counter end to end (§3) — ladder (unless given), one pairings_pt_run,
+    estimate.  Needs torch for the device counters unless `device_alloc(n_uint64) -> (ptr, read)` is given.
+    Returns dict(identified, distinct, betas, ratios, moves, swaps, samples)."""
+    import math
+    import torch
+    if betas is None:
+        betas = pairings_pt_ladder(kind, n, target_exchange, 256, 1 << (14 if n <= 16 else 18), seed ^ 0x5bd1e995)
+    if burn_in is None:
+        burn_in = iterations // 2
+    M, N = len(betas), 2 * n
+    hist = torch.zeros((M, N + 1), dtype=torch.int64, device="cuda")
+    mv = torch.zeros(M, dtype=torch.int64, device="cuda")
+    sw = torch.zeros(M, dtype=torch.int64, device="cuda")
+    done = 0
+    while done < replicas:                          # at most 2^30 replicas and 2^25 iterations per call
+        take = min(replicas - done, 1 << 20)
+        pairings_pt_run(kind, n, betas, done, done + take, iterations, burn_in, seed, hist.data_ptr(), mv.data_ptr(),
+                        sw.data_ptr(), torch.cuda.current_stream().cuda_stream)
+        done += take
+    torch.cuda.synchronize()
+    h = hist.cpu().tolist()
+    ratios, logz = pairings_pt_estimate(kind, n, betas, h)
+    return dict(distinct=math.exp(logz), identified=math.exp(logz) / 2, betas=betas, ratios=ratios,
+                moves=mv.cpu().tolist(), swaps=sw.cpu().tolist(), samples=replicas * (iterations - burn_in))
 
 
 def default_chunk_bits(n: int) -> int:

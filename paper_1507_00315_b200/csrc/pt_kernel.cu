@@ -215,6 +215,71 @@ int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
     return PAIRINGS_OK;
 }
 
+// Ladder choice ("the inverse temperatures are chosen such that the acceptance rates for the
+// configuration exchanges are no smaller than one half", with as few levels as that allows).  Built level by
+// level: a short pilot run of the ladder so far gives the energy distribution p(E) of its last level; the next
+// beta is the one for which the predicted exchange acceptance
+//     A(db) = sum_{E,E'} p(E) q(E') min[1, exp(-db (E - E'))],   q(E') ~ p(E') exp(-db E')   (p reweighted to beta + db)
+// equals the target (bisection; A falls from 1 as db grows; at most a doubling of beta per level).  Stops when the
+// last level sits at E = 0 with probability >= 0.98 or beta >= 32 (the remaining factor to beta = infinity is ~1).
+int pairings_pt_ladder(int kind, int n, double target_exchange, uint64_t pilot_replicas, uint64_t pilot_iterations,
+                       uint64_t seed, double* betas_out, int cap_levels, void* stream) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    if (!betas_out) return PAIRINGS_ENULL;
+    if (!(target_exchange > 0.05 && target_exchange < 0.95) || cap_levels < 1 || pilot_replicas == 0 ||
+        pilot_iterations < 2 || pilot_iterations > (1ULL << 25)) return PAIRINGS_EINVAL_OPTS;
+    const int N = 2 * n, cap = cap_levels < PAIRINGS_PT_MAX_LEVELS ? cap_levels : PAIRINGS_PT_MAX_LEVELS;
+    cudaStream_t s = (cudaStream_t)stream;
+    std::vector<double> betas(1, 0.0);
+    const size_t words = (size_t)PAIRINGS_PT_MAX_LEVELS * (size_t)(N + 1) + 2 * PAIRINGS_PT_MAX_LEVELS;
+    uint64_t* dev = nullptr;
+    (void)cudaGetLastError();
+    if (cudaMallocAsync((void**)&dev, words * sizeof(uint64_t), s) != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    std::vector<uint64_t> host(words);
+    int result = PAIRINGS_ERANGE;                                      // cap reached before the ladder is cold enough
+    for (;;) {
+        const int M = (int)betas.size();
+        cudaError_t e = cudaMemsetAsync(dev, 0, words * sizeof(uint64_t), s);
+        if (e != cudaSuccess) { result = PAIRINGS_ECUDA; break; }
+        rc = pairings_pt_run(kind, n, betas.data(), M, 0, pilot_replicas, pilot_iterations, pilot_iterations / 2,
+                             seed + (uint64_t)M, dev, dev + (size_t)PAIRINGS_PT_MAX_LEVELS * (N + 1),
+                             dev + (size_t)PAIRINGS_PT_MAX_LEVELS * (N + 1) + PAIRINGS_PT_MAX_LEVELS, s);
+        if (rc) { result = rc; break; }
+        e = cudaMemcpyAsync(host.data(), dev, words * sizeof(uint64_t), cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        if (e != cudaSuccess) { result = PAIRINGS_ECUDA; break; }
+        std::vector<double> pE((size_t)N + 1);
+        double tot = 0;
+        for (int E = 0; E <= N; E++) { pE[E] = (double)host[(size_t)(M - 1) * (N + 1) + E]; tot += pE[E]; }
+        for (int E = 0; E <= N; E++) pE[E] /= tot;
+        if (pE[0] >= 0.98 || betas.back() >= 32.0) { result = M; break; }   // cold enough: the factor to beta = infinity is ~1
+        if (M == cap) break;
+        auto acceptance = [&](double db) {
+            std::vector<double> q((size_t)N + 1);
+            double z = 0;
+            for (int E = 0; E <= N; E++) { q[E] = pE[E] * std::exp(-db * E); z += q[E]; }
+            double a = 0;
+            for (int E = 0; E <= N; E++)
+                for (int F = 0; F <= N; F++)
+                    a += pE[E] * (q[F] / z) * (E <= F ? 1.0 : std::exp(-db * (double)(E - F)));
+            return a;
+        };
+        // at most a doubling per level (the cold end of Table 6 goes 8.1, 16, 32): with only E in {0, 1} left the
+        // predicted acceptance no longer falls to the target
+        double lo = 0.0, hi = betas.back() > 1.0 ? betas.back() : 1.0;
+        for (int it = 0; it < 60; it++) {
+            const double mid = 0.5 * (lo + hi);
+            if (acceptance(mid) > target_exchange) lo = mid; else hi = mid;
+        }
+        betas.push_back(betas.back() + 0.5 * (lo + hi));
+    }
+    cudaError_t e2 = cudaFreeAsync(dev, s);
+    cudaError_t e3 = cudaStreamSynchronize(s);
+    if (result > 0 && (e2 != cudaSuccess || e3 != cudaSuccess)) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    if (result > 0) for (int j = 0; j < result; j++) betas_out[j] = betas[(size_t)j];
+    return result;
+}
+
 int pairings_pt_estimate(int kind, int n, const double* betas, int n_levels, const uint64_t* hist_host,
                          double* ratios_out, double* log_distinct_out) {
     int rc = pt_check(kind, n, betas, n_levels); if (rc) return rc;

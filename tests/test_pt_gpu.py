@@ -74,3 +74,17 @@ def test_table6_ladder_estimates_s12_within_one_percent():
     ratios, logz = pb.pairings_pt_estimate(S, 12, betas, hist)
     est = math.exp(logz) / 2
     assert abs(est - 227968) < 0.01 * 227968, est
+
+
+@pytest.mark.parametrize("kind,n,exact", [(S, 12, 227968), (S, 16, 700078384), (L, 12, 108144)])
+def test_ladder_gives_half_exchange_rates_and_a_good_estimate(kind, n, exact):
+    # exchange acceptance "no smaller than one half"; Tables 7/8: approximate within ~1 % of the exact count
+    betas = pb.pairings_pt_ladder(kind, n, 0.55, 256, 1 << 14, 7)
+    assert betas[0] == 0.0 and all(b > a for a, b in zip(betas, betas[1:])) and 6 <= len(betas) <= 20
+    assert betas == pb.pairings_pt_ladder(kind, n, 0.55, 256, 1 << 14, 7)            # deterministic
+    r = pb.approx_count(kind, n, 1 << 12, 1 << 16, betas=betas)
+    rates = [s / r["samples"] for s in r["swaps"][:-1]]
+    assert all(x >= 0.5 for x in rates), rates
+    assert abs(r["identified"] - exact) < 0.025 * exact, r["identified"]
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_pt_ladder(kind, n, 0.55, 256, 1 << 14, 7, cap_levels=3)          # cap reached first
