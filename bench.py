@@ -173,11 +173,16 @@ class ClockSampler:
         for ln in self.proc.stdout:
             self.lines.append((time.perf_counter(), ln.strip()))
 
-    def stop(self, t0, t1):
+    def close(self):
+        if self.proc is not None:
+            self.proc.terminate()
+
+    def window(self, t0, t1):
+        """Clock statistics of the samples taken in [t0, t1] (the sampler keeps running: starting nvidia-smi
+        inside or right before a wall-clock region would perturb it)."""
         if self.proc is None:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
         time.sleep(0.25)
-        self.proc.terminate()
         sm, mx, reasons = [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for t, ln in self.lines:
@@ -259,6 +264,9 @@ def run_gpu(args):
             assert S == L20_IDENTIFIED and D == 2 * S, ("L(20) mismatch", D, S)
         return total
 
+    sampler = ClockSampler(local)          # one nvidia-smi for the whole run, started well before the timed regions
+    sampler.start()
+
     # ---- warm-up (>= 3), correctness of the warmed-up path
     for _ in range(max(args.warmup, 3) if args.warmup >= 0 else 3):
         step_device()
@@ -276,9 +284,6 @@ def run_gpu(args):
     phi = float(nzt.item()) / terms_rank
 
     # ---- timed: K steps, CUDA events per step on the launching stream, L2 flushed between steps
-    sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.3)
     barrier()
     t_begin = time.perf_counter()
     evs = []
@@ -291,7 +296,7 @@ def run_gpu(args):
         flush.fill_(1)
     barrier()
     t_end = time.perf_counter()
-    clocks = sampler.stop(t_begin, t_end)
+    clocks = sampler.window(t_begin, t_end)
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
     if dist is not None:
         t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
@@ -304,9 +309,6 @@ def run_gpu(args):
     # ---- e2e: the public host-buffer call, wall clock, copies + allocation inside
     for _ in range(2):
         pb.count_pairings_host(kind, n, C, begin, end, moduli, stream, opts, out=host_ptr)
-    sampler2 = ClockSampler(local)
-    sampler2.start()
-    time.sleep(0.3)
     barrier()
     t0 = time.perf_counter()
     for _ in range(args.steps):
@@ -314,7 +316,8 @@ def run_gpu(args):
         finish(host_rows)
     barrier()
     e2e_s = time.perf_counter() - t0
-    clocks_e2e = sampler2.stop(t0, t0 + e2e_s)
+    clocks_e2e = sampler.window(t0, t0 + e2e_s)
+    sampler.close()
     if dist is not None:
         t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)

@@ -110,8 +110,9 @@ int count_pairings_ex(int kind, int n, int chunk_bits,
 /* 1 if PAIRINGS_VARIANT_SWAR is compiled for (kind, n), else 0. */
 int pairings_has_swar(int kind, int n);
 
-/* Same computation with a HOST output buffer: allocates the device rows on `stream`
- * (cudaMallocAsync), launches, copies the rows back and synchronises the stream.  This is the
+/* Same computation with a HOST output buffer: allocates the device rows on `stream` from a memory pool of the
+ * library's own (one per device, created on first use, keeps at most 64 MiB between calls — the only device
+ * memory the library ever retains), launches, copies the rows back and synchronises the stream.  This is the
  * end-to-end call bench.py times as "e2e".  out_residues_host: (chunk_end-chunk_begin)*n_moduli. */
 int count_pairings_host(int kind, int n, int chunk_bits,
                         uint64_t chunk_begin, uint64_t chunk_end,

@@ -20,6 +20,7 @@
 #include <algorithm>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -225,6 +226,31 @@ static int validate(int kind, int n, int chunk_bits, uint64_t b, uint64_t e, con
     return PAIRINGS_OK;
 }
 
+// One memory pool per device for count_pairings_host's staging rows (created on first use, never destroyed).
+static cudaMemPool_t staging_pool() {
+    static std::mutex mu;
+    static cudaMemPool_t pools[64] = {};
+    static bool tried[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) { (void)cudaGetLastError(); return nullptr; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!tried[dev]) {
+        tried[dev] = true;
+        cudaMemPoolProps props; std::memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t p = nullptr;
+        if (cudaMemPoolCreate(&p, &props) == cudaSuccess) {
+            unsigned long long keep = 64ULL << 20;
+            (void)cudaMemPoolSetAttribute(p, cudaMemPoolAttrReleaseThreshold, &keep);
+            pools[dev] = p;
+        } else (void)cudaGetLastError();
+    }
+    return pools[dev];
+}
+
 static int launch_range(int kind, int n, int chunk_bits, uint64_t chunk_begin, uint64_t chunk_end,
                         const uint32_t* moduli, int n_moduli, uint32_t* out, cudaStream_t stream,
                         const pairings_launch_opts* opts) {
@@ -297,7 +323,12 @@ int count_pairings_host(int kind, int n, int chunk_bits, uint64_t chunk_begin, u
     const size_t bytes = n_chunks * (size_t)n_moduli * sizeof(uint32_t);
     uint32_t* dev = nullptr;
     (void)cudaGetLastError();
-    if (cudaMallocAsync((void**)&dev, bytes, s) != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    // The staging rows come from a pool of the library's own that keeps up to 64 MiB between calls: with the
+    // default pool (release threshold 0) every synchronise hands the memory back to the driver, and the next
+    // call's allocation was measured to cost up to 0.5 s.
+    cudaMemPool_t pool = staging_pool();
+    cudaError_t ea = pool ? cudaMallocFromPoolAsync((void**)&dev, bytes, pool, s) : cudaMallocAsync((void**)&dev, bytes, s);
+    if (ea != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
     rc = launch_range(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, dev, s, opts);
     cudaError_t e1 = cudaSuccess;
     if (rc == PAIRINGS_OK) e1 = cudaMemcpyAsync(out_residues_host, dev, bytes, cudaMemcpyDeviceToHost, s);
