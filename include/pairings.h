@@ -107,6 +107,15 @@ int count_pairings_ex(int kind, int n, int chunk_bits,
                       uint32_t* out_residues, void* stream,
                       const pairings_launch_opts* opts /* HOST, may be NULL */);
 
+/* The launch geometry count_pairings_ex would use for a call over `n_chunks` chunks (chunk_end - chunk_begin) with
+ * these options: kernel variant, Gray bits g per thread prefix, threads per block, blocks per chunk.
+ * The geometry depends on n_chunks (few chunks are spread over several blocks each), so a test that wants the
+ * geometry of a large launch on a small one asks here and pins the answer in `opts`.  Host only, launches
+ * nothing.  Any *_out may be NULL.  Errors as count_pairings_ex (PAIRINGS_EINVAL_OPTS: options not satisfiable). */
+int pairings_query_geometry(int kind, int n, int chunk_bits, uint64_t n_chunks,
+                            const pairings_launch_opts* opts /* HOST, may be NULL */,
+                            int* variant_out, int* gray_bits_out, int* block_threads_out, int* blocks_per_chunk_out);
+
 /* 1 if PAIRINGS_VARIANT_SWAR is compiled for (kind, n), else 0. */
 int pairings_has_swar(int kind, int n);
 

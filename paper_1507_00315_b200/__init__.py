@@ -6,7 +6,7 @@ fallback: importing works without a GPU, compute calls raise PairingsError(PAIRI
 from .api import (  # noqa: F401
     SKOLEM, LANGFORD, VARIANT_AUTO, VARIANT_GENERIC, VARIANT_SWAR,
     PairingsError, LaunchOpts, lib, library_path,
-    count_pairings, count_pairings_ex, count_pairings_host, pairings_has_swar,
+    count_pairings, count_pairings_ex, count_pairings_host, pairings_has_swar, pairings_query_geometry,
     pairings_default_moduli, pairings_min_moduli, pairings_bound_moduli,
     pairings_partition, pairings_rank_range, pairings_sum_rows,
     pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_lemma24, RUN_LEMMA24, RUN_DUPLICATE,

@@ -51,6 +51,8 @@ def lib():
         "count_pairings_ex": (i, [i, i, i, u64, u64, u32p, i, vp, vp, optp]),
         "count_pairings_host": (i, [i, i, i, u64, u64, u32p, i, u32p, vp, optp]),
         "pairings_has_swar": (i, [i, i]),
+        "pairings_query_geometry": (i, [i, i, i, u64, optp, ctypes.POINTER(i), ctypes.POINTER(i), ctypes.POINTER(i),
+                                        ctypes.POINTER(i)]),
         "pairings_default_moduli": (i, [u32p, i]),
         "pairings_min_moduli": (i, [i, i]),
         "pairings_bound_moduli": (i, [i, i]),
@@ -103,6 +105,14 @@ def pairings_build_info() -> str:
 
 def pairings_has_swar(kind: int, n: int) -> bool:
     return bool(lib().pairings_has_swar(kind, n))
+
+
+def pairings_query_geometry(kind, n, chunk_bits, n_chunks, opts: Optional[LaunchOpts] = None):
+    """(variant, gray_bits, block_threads, blocks_per_chunk) of a count_pairings_ex call over n_chunks chunks."""
+    v, g, t, b = ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int(0), ctypes.c_int(0)
+    _check(lib().pairings_query_geometry(kind, n, chunk_bits, n_chunks, _opts(opts), ctypes.byref(v), ctypes.byref(g),
+                                         ctypes.byref(t), ctypes.byref(b)), "pairings_query_geometry")
+    return int(v.value), int(g.value), int(t.value), int(b.value)
 
 
 def count_pairings(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, out_residues_ptr: int, stream: int = 0):

@@ -305,6 +305,19 @@ int count_pairings(int kind, int n, int chunk_bits, uint64_t chunk_begin, uint64
     return count_pairings_ex(kind, n, chunk_bits, chunk_begin, chunk_end, moduli, n_moduli, out_residues, stream, nullptr);
 }
 
+int pairings_query_geometry(int kind, int n, int chunk_bits, uint64_t n_chunks, const pairings_launch_opts* opts,
+                            int* variant_out, int* gray_bits_out, int* block_threads_out, int* blocks_per_chunk_out) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
+    if (n_chunks == 0 || (chunk_bits < 64 && n_chunks > (1ULL << chunk_bits))) return PAIRINGS_EINVAL_CHUNK;
+    Geometry geo; rc = choose_geometry(kind, n, chunk_bits, n_chunks, opts, &geo); if (rc) return rc;
+    if (variant_out) *variant_out = geo.variant;
+    if (gray_bits_out) *gray_bits_out = geo.g;
+    if (block_threads_out) *block_threads_out = geo.threads;
+    if (blocks_per_chunk_out) *blocks_per_chunk_out = 1 << geo.log2_bpc;
+    return PAIRINGS_OK;
+}
+
 int pairings_has_swar(int kind, int n) {
     if (check_kind_n(kind, n)) return 0;
     return swar_lookup(kind, n) != nullptr ? 1 : 0;

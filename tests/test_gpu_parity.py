@@ -235,19 +235,47 @@ def test_lemma24_refuses_a_journal_of_the_other_half(tmp_path):
     assert e.value.code == -11
 
 
-# ---- BASELINE configs 4 and 5 at full size, in the launch configuration bench.py times: rows of seeded
-# chunks against the oracle one by one (each oracle chunk is 2^23 .. 2^27 plain evaluations).
+# ---- BASELINE configs 4 and 5 at full size: rows of seeded chunks against the oracle one by one (each oracle
+# chunk is 2^23 .. 2^27 plain evaluations), in the launch geometry bench.py times.  The geometry depends on the
+# number of chunks of a launch, so the test asks pairings_query_geometry for the geometry of the bench's launch
+# (bench.WL: all 2^16 chunks of L(20) in one call; bench.OTHER_CONFIGS: all 2^18 chunks of S(21); bench.WL24: runs of
+# 1024 chunks of S(24)) and pins it on the small launches around the sampled chunks.
+def bench_launch_chunks(kind, n, C):
+    import bench
+    if (kind, n, C) == (bench.WL["kind"], bench.WL["n"], bench.WL["chunk_bits"]):
+        return 1 << C
+    if (kind, n, C) == (bench.WL24["kind"], bench.WL24["n"], bench.WL24["chunk_bits"]):
+        return bench.WL24["run_len"]
+    assert any((k, nn, cc) == (kind, n, C) for (k, nn, cc, _m, _r, _w) in bench.OTHER_CONFIGS)
+    return 1 << C
+
+
 @pytest.mark.parametrize("kind,n,C,m,count", [(L, 20, 16, 7, 16), (S, 21, 18, 7, 16), (S, 24, 20, 9, 4)])
 def test_full_size_sampled_chunks_match_oracle(kind, n, C, m, count):
     moduli = pb.pairings_default_moduli(m)
     chunks = seeds.sample_chunks(C, count, salt=100 + n)
     want = oracle_rows(kind, n, C, chunks, moduli, threads=16, pieces=16 if n == 24 else 1)
-    # the bench launches whole ranges: take each sampled chunk out of a 64-chunk launch around it
-    for c, w in zip(chunks, want):
+    v, g, t, bpc = pb.pairings_query_geometry(kind, n, C, bench_launch_chunks(kind, n, C))
+    assert v == pb.VARIANT_SWAR
+    pinned = pb.LaunchOpts(variant=v, gray_bits=g, block_threads=t, blocks_per_chunk=bpc)
+    assert pb.pairings_query_geometry(kind, n, C, 8, pinned) == (v, g, t, bpc)       # the pin holds on a small launch
+    for i, (c, w) in enumerate(zip(chunks, want)):
+        b = min(c & ~7, (1 << C) - 8)
+        rows = gpu_rows(kind, n, C, b, b + 8, moduli, pb.LaunchOpts(variant=v, gray_bits=g, block_threads=t, blocks_per_chunk=bpc))
+        assert rows[c - b] == w[2], (kind, n, c, "bench geometry", g, t, bpc)
+        assert pb.pairings_crt_signed(moduli, rows[c - b]) == w[0]
+        # the library's own choice for a 64-chunk launch (several blocks per chunk, atomic mod-add of the block sums)
         b = min(c & ~63, (1 << C) - 64)
         rows = gpu_rows(kind, n, C, b, b + 64, moduli)
-        assert rows[c - b] == w[2], (kind, n, c)
-        assert pb.pairings_crt_signed(moduli, rows[c - b]) == w[0]
+        assert rows[c - b] == w[2], (kind, n, c, "default geometry")
+        if i < 4:
+            # every other Gray-bit count the outer-flip dispatch of this instance has (per-row, not through a sum)
+            for g2 in range(max(g - 3, 5), min(n - 2, 16) + 1):
+                for bpc2 in (1, 4):
+                    if 2 * n - 1 - C - g2 < (t * bpc2).bit_length() - 1:
+                        continue                                       # fewer prefixes than threads
+                    o = pb.LaunchOpts(variant=v, gray_bits=g2, block_threads=t, blocks_per_chunk=bpc2)
+                    assert gpu_rows(kind, n, C, c, c + 1, moduli, o)[0] == w[2], (kind, n, c, g2, bpc2)
 
 
 @pytest.mark.parametrize("kind,n,C", [(L, 20, 16), (S, 20, 16), (S, 21, 18)])
