@@ -46,10 +46,10 @@ namespace swar {
 
 constexpr int H = PAIRINGS_SWAR_H;              // unrolled inner Gray bits
 constexpr int BLK = 1 << H;       // steps per unrolled block
-constexpr int QCAP = 256;         // ring entries per warp (power of two)
-constexpr int QUAD = 4;           // steps between drain checks; 31 + 32*QUAD < QCAP
-constexpr int PLANE_BYTES = QCAP * 16;   // ring = planes of 16 bytes per entry (conflict-free 128-bit accesses)
-constexpr int RING_ALIGN = PLANE_BYTES;  // plane 0 of every ring is PLANE_BYTES-aligned: slot address = ring | offset
+constexpr int QUAD = 4;           // steps per slot allocation and between drain checks
+constexpr int SCAP = 160;         // stack entries per warp: at most 31 left by the last drain + 32 * QUAD of one quad
+constexpr int PLANE_BYTES = SCAP * 16;   // stack = planes of 16 bytes per entry (128-bit accesses)
+static_assert(31 + 32 * QUAD < SCAP && 32 * QUAD <= 255, "stack capacity; per-quad lane prefixes are scanned in byte fields");
 
 #define PAIRINGS_HD __host__ __device__ constexpr
 
@@ -390,6 +390,19 @@ __device__ __forceinline__ void sts_v1_clr(uint32_t addr, uint32_t a, uint32_t w
     asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %2, %3;\n\tsetp.eq.u32 p, t, 0;\n\t@p st.shared.u32 [%0], %1;\n\t}"
                  :: "r"(addr), "r"(a), "r"(word), "r"(bit) : "memory");
 }
+// slot += 16 iff (word & bit) == 0 — the same predicate as the stores of that step
+__device__ __forceinline__ void add16_clr(uint32_t& slot, uint32_t word, uint32_t bit) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.eq.u32 p, t, 0;\n\t@p add.u32 %0, %0, 16;\n\t}"
+                 : "+r"(slot) : "r"(word), "r"(bit));
+}
+// one Kogge-Stone step of an inclusive scan over the lanes, two words at a time (byte fields that cannot overflow)
+template <int D>
+__device__ __forceinline__ void scan_up2(uint32_t& a, uint32_t& b) {
+    asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t, u;\n\t"
+                 "shfl.sync.up.b32 t|p, %0, %2, 0, 0xffffffff;\n\t"
+                 "shfl.sync.up.b32 u, %1, %2, 0, 0xffffffff;\n\t"
+                 "@p add.u32 %0, %0, t;\n\t@p add.u32 %1, %1, u;\n\t}" : "+r"(a), "+r"(b) : "n"(D));
+}
 __device__ __forceinline__ void lds_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
 }
@@ -402,7 +415,23 @@ __device__ __forceinline__ int sbyte(uint32_t w) {
     return (int)r;
 }
 
-// One ring entry (at shared byte address `addr` in plane 0) -> signed multi-word term -> acc.
+// signed 32 x 32 -> 64 (+ 64) as ONE IMAD.WIDE each; hi / lo words of a 64-bit value
+__device__ __forceinline__ long long mulw(int a, int b) { long long r; asm("mul.wide.s32 %0, %1, %2;" : "=l"(r) : "r"(a), "r"(b)); return r; }
+__device__ __forceinline__ long long madw(int a, int b, long long c) { long long r; asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c)); return r; }
+__device__ __forceinline__ void split64(long long v, uint32_t& lo, uint32_t& hi) { asm("mov.b64 {%0, %1}, %2;" : "=r"(lo), "=r"(hi) : "l"(v)); }
+// signed digits of a 64-bit value: v = d1 * 2^32 + d0 with d0 = (int) low word
+__device__ __forceinline__ void digits64(long long v, int& d0, int& d1) {
+    uint32_t lo, hi; split64(v, lo, hi);
+    d0 = (int)lo; d1 = (int)(hi + (lo >> 31));
+}
+// v >> 32 (arithmetic) as a 64-bit value: the sign-extended upper half
+__device__ __forceinline__ long long upper64(long long v) {
+    uint32_t lo, hi; split64(v, lo, hi);
+    long long r; asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "r"(hi), "r"((uint32_t)((int)hi >> 31)));
+    return r;
+}
+
+// One stack entry (at shared byte address `addr` in plane 0) -> signed multi-word term -> acc.
 template <int KIND, int NN>
 __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<KIND, NN>::W], uint32_t c80) {
     using L = Lay<KIND, NN>;
@@ -449,40 +478,28 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<K
         }
     });
     if constexpr (G <= 4) {
-        // signed multi-word product T = gp[0] * gp[1] * ... (two's complement, top word signed).  A k-word T
-        // times a signed 32-bit m: the k-1 low (unsigned) words are multiplied by m read as unsigned, i.e.
-        // by m + 2^32 [m < 0], and that excess — the low words shifted up one word — is subtracted again.
+        // signed multi-word product T = gp[0] * gp[1] * ... (two's complement, top word signed) from signed 64-bit
+        // pieces only: a 64-bit product A = a1 * 2^32 + a0 is split with a SIGNED low digit a0 = (int) low word,
+        // a1 = high word + bit 31 of the low word, so every partial product is one signed IMAD.WIDE whose 64-bit
+        // addend carries the sign-extended upper half of the digit below — no unsigned-times-signed corrections.
         uint32_t T[W];
-#pragma unroll
-        for (int i = 0; i < W; i++) T[i] = 0;
-        T[0] = (uint32_t)gp[0];
-        static_for<1, G>([&](auto gc) {
-            PAIRINGS_IC(k, gc);                                   // T has k words before this multiplication
-            const int m = gp[k];
-            uint32_t lowT[k > 1 ? k - 1 : 1];
-            uint32_t carry = 0;
-            static_for<0, k - 1>([&](auto ic) {
-                PAIRINGS_IC(i, ic);
-                lowT[i] = T[i];
-                const uint64_t p = (uint64_t)T[i] * (uint32_t)m + carry;
-                T[i] = (uint32_t)p; carry = (uint32_t)(p >> 32);
-            });
-            int64_t top;                                          // signed top word x signed m + carry: one IMAD.WIDE
-            asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(top) : "r"((int)T[k - 1]), "r"(m), "l"((int64_t)(uint64_t)carry));
-            T[k - 1] = (uint32_t)(uint64_t)top; T[k] = (uint32_t)((uint64_t)top >> 32);
-            if constexpr (k == 2) {
-                asm("{\n\t.reg .pred p;\n\tsetp.lt.s32 p, %3, 0;\n\t@p sub.cc.u32 %0, %0, %2;\n\t@p subc.u32 %1, %1, 0;\n\t}"
-                    : "+r"(T[1]), "+r"(T[2]) : "r"(lowT[0]), "r"(m));
-            } else if constexpr (k == 3) {
-                asm("{\n\t.reg .pred p;\n\tsetp.lt.s32 p, %5, 0;\n\t@p sub.cc.u32 %0, %0, %3;\n\t@p subc.cc.u32 %1, %1, %4;\n\t@p subc.u32 %2, %2, 0;\n\t}"
-                    : "+r"(T[1]), "+r"(T[2]), "+r"(T[3]) : "r"(lowT[0]), "r"(lowT[1]), "r"(m));
-            } else if constexpr (k == 4) {
-                asm("{\n\t.reg .pred p;\n\tsetp.lt.s32 p, %7, 0;\n\t@p sub.cc.u32 %0, %0, %4;\n\t@p subc.cc.u32 %1, %1, %5;\n\t@p subc.cc.u32 %2, %2, %6;\n\t@p subc.u32 %3, %3, 0;\n\t}"
-                    : "+r"(T[1]), "+r"(T[2]), "+r"(T[3]), "+r"(T[4]) : "r"(lowT[0]), "r"(lowT[1]), "r"(lowT[2]), "r"(m));
-            } else {
-                static_assert(k == 1, "more than 5 groups: extend the correction chain");
-            }
-        });
+        if constexpr (G == 1) {
+            T[0] = (uint32_t)gp[0];
+        } else if constexpr (G == 2) {
+            split64(mulw(gp[0], gp[1]), T[0], T[1]);
+        } else if constexpr (G == 3) {
+            int a0, a1; digits64(mulw(gp[0], gp[1]), a0, a1);                   // |A| < 2^62
+            const long long X = mulw(a0, gp[2]);
+            const long long Y = madw(a1, gp[2], upper64(X));
+            uint32_t xh; split64(X, T[0], xh); split64(Y, T[1], T[2]);
+        } else {
+            int a0, a1, b0, b1;
+            digits64(mulw(gp[0], gp[1]), a0, a1); digits64(mulw(gp[2], gp[3]), b0, b1);
+            const long long X = mulw(a0, b0);
+            const long long Y = madw(a0, b1, madw(a1, b0, upper64(X)));          // |a1 b0|, |a0 b1| <= 2^61
+            const long long Z = madw(a1, b1, upper64(Y));
+            uint32_t xh, yh; split64(X, T[0], xh); split64(Y, T[1], yh); split64(Z, T[2], T[3]);
+        }
         const uint32_t sext = (uint32_t)((int)T[G - 1] >> 31);    // sign words above the G-word product
 #pragma unroll
         for (int i = G; i < W; i++) T[i] = sext;
@@ -526,13 +543,19 @@ struct Walker {
     uint32_t C[H][NR];
     uint32_t E, O;            // de-interleaved sign word: E bit i = index bit 2i, O bit i = index bit 2i+1
     uint32_t acc[W];
-    uint32_t tail16, head16;  // warp-uniform ring counters (monotone), in units of 1/16 entry (= byte offsets)
-    uint32_t ltmask;
-    uint32_t ring;            // shared-window byte address of this warp's ring (plane 0), RING_ALIGN-aligned
+    // Non-zero terms go to a per-warp STACK in shared memory (the sum is commutative: any lane may multiply any
+    // entry, in any order).  top = shared byte address (plane 0) of the first free entry, warp-uniform.
+    uint32_t top;
+    uint32_t lim;             // stack base + 32 entries: a full drain round is possible while top >= lim
     uint32_t lane16;          // lane * 16
     uint32_t c80;             // 0x80808080 (KernelParams::c80)
     uint32_t Vo;              // outer sign word: bit i = index bit H + i (set <-> x = -1)
     uint32_t ZM;              // zero-step mask of the current block: bit S set <-> the term of step S has a zero factor
+    // Slot plan of the current block, from ZM alone (known before the first step): byte j of ex[w] = number of
+    // non-zero steps of quad 2j+w in the lanes below this one, byte j of tot[w] = that count over the whole warp.
+    uint32_t ex[2], tot[2];
+    uint32_t slot;            // this lane's next free entry of the current quad (lane-major inside a quad)
+    uint32_t nzc;             // non-zero terms pushed by the warp (warp-uniform, 32-bit: reset per prefix)
 
     // Row a4 for the whole block: OR over the even-distance slots of the table masks (see ztab above).
     __device__ __forceinline__ void zero_mask() {
@@ -557,46 +580,53 @@ struct Walker {
             zm |= mask;
         });
         ZM = zm;
+        // ---- slot plan: per-lane counts of the non-zero steps of each quad (nibble popcounts of ~ZM), then an
+        // inclusive scan over the lanes in byte fields (a field is at most 4 * 32 = 128)
+        const uint32_t nzm = ~zm;
+        uint32_t x = nzm - ((nzm >> 1) & 0x55555555u);
+        x = (x & 0x33333333u) + ((x >> 2) & 0x33333333u);                  // nibble q = steps 4q .. 4q+3
+        const uint32_t c0 = x & 0x0F0F0F0Fu, c1 = (x >> 4) & 0x0F0F0F0Fu;   // byte j of c0: quad 2j, of c1: quad 2j+1
+        uint32_t s0 = c0, s1 = c1;
+        scan_up2<1>(s0, s1); scan_up2<2>(s0, s1); scan_up2<4>(s0, s1); scan_up2<8>(s0, s1); scan_up2<16>(s0, s1);
+        ex[0] = s0 - c0; ex[1] = s1 - c1;                                  // no borrow: s >= c in every byte
+        // warp totals by REDUX (a byte sum is at most 128: no carry between fields): provably warp-uniform, which the
+        // stack pointer and every drain loop inherit — the compiler then knows the warp stays converged
+        tot[0] = __reduce_add_sync(0xffffffffu, c0); tot[1] = __reduce_add_sync(0xffffffffu, c1);
+        nzc = __dp4a(tot[0], 0x01010101u, __dp4a(tot[1], 0x01010101u, nzc));
     }
 
     template <int S>
     __device__ __forceinline__ void push_if_nonzero() {
         constexpr uint32_t bit = 1u << S;
-        const uint32_t bal = __ballot_sync(0xffffffffu, (ZM & bit) == 0);
-        // slot = (tail + rank among the warp's non-zero lanes) mod QCAP; ring is aligned, so "|" adds the offset
-        const uint32_t addr = ((tail16 + 16u * (uint32_t)__popc(bal & ltmask)) & (uint32_t)(PLANE_BYTES - 16)) | ring;
-        // entry words: Q[0..NR), sign; plane p holds words 4p..4p+3 (predicated vector stores, no branch)
+        // entry words: Q[0..NR); plane p holds words 4p..4p+3 (predicated vector stores, no branch)
         uint32_t e[4 * L::PLANES];
 #pragma unroll
         for (int i = 0; i < 4 * L::PLANES; i++) e[i] = Q[i < NR ? i : 0];
         static_for<0, L::PLANES>([&](auto pc) {
             PAIRINGS_IC(pl, pc);
             constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
-            if constexpr (words >= 3) sts_v4_clr(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
-            else if constexpr (words == 2) sts_v2_clr(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
-            else sts_v1_clr(addr + pl * PLANE_BYTES, e[4 * pl], ZM, bit);
+            if constexpr (words >= 3) sts_v4_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
+            else if constexpr (words == 2) sts_v2_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
+            else sts_v1_clr(slot + pl * PLANE_BYTES, e[4 * pl], ZM, bit);
         });
-        tail16 += 16u * (uint32_t)__popc(bal);
-    }
-
-    __device__ __forceinline__ uint32_t slot_of_lane() const {
-        return ((head16 + lane16) & (uint32_t)(PLANE_BYTES - 16)) | ring;
+        if constexpr (S % QUAD != QUAD - 1) add16_clr(slot, ZM, bit);
     }
 
     __device__ __forceinline__ void drain_full() {
-        while (tail16 - head16 >= 32u * 16u) {
+        while (top >= lim) {                                   // warp-uniform
+            top -= 32u * 16u;
             __syncwarp();
-            drain_entry<KIND, NN>(slot_of_lane(), acc, c80);
-            head16 += 32u * 16u;
+            drain_entry<KIND, NN>(top + lane16, acc, c80);
             __syncwarp();
         }
     }
 
     __device__ __forceinline__ void drain_rest() {
         drain_full();
+        const uint32_t base = lim - 32u * 16u;
         __syncwarp();
-        if (lane16 < tail16 - head16) drain_entry<KIND, NN>(slot_of_lane(), acc, c80);
-        head16 = tail16;
+        if (lane16 < top - base) drain_entry<KIND, NN>(base + lane16, acc, c80);
+        top = base;
         __syncwarp();
     }
 
@@ -604,11 +634,14 @@ struct Walker {
     // current term, then flip inner bit ctz(S+1) (the block's last step is followed by block_end).
     template <int QI>
     __device__ __forceinline__ void quad() {
+        constexpr uint32_t sel16 = 16u << (8 * (QI >> 1));                 // 16 * byte (QI >> 1) of word (QI & 1)
+        slot = __dp4a(ex[QI & 1], sel16, top);
         static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
             PAIRINGS_IC(S, sc);
             push_if_nonzero<S>();
             if constexpr (S + 1 < BLK) inner_flip<zbits(S), ctz_c(S + 1)>();
         });
+        top = __dp4a(tot[QI & 1], sel16, top);
     }
 
     // flip of inner bit bi in inner state ZB: dQ = -x_j * C[bi] + K  (row a3; K = inner neighbours, folded)
@@ -699,12 +732,11 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     constexpr int N = L::N, B = N - 1, W = L::W;
     extern __shared__ uint32_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // dynamic shared memory: [alignment slack][rings: warps x PLANES x PLANE_BYTES][reduction scratch]
-    const uint32_t smem_base = (uint32_t)__cvta_generic_to_shared(smem);
-    const uint32_t rings = (smem_base + (uint32_t)(RING_ALIGN - 1)) & ~(uint32_t)(RING_ALIGN - 1);
-    const uint32_t ring_bytes = (blockDim.x >> 5) * (uint32_t)(L::PLANES * PLANE_BYTES);
+    // dynamic shared memory (16-byte aligned): [stacks: warps x PLANES x PLANE_BYTES][reduction scratch]
+    const uint32_t stacks = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t stack_bytes = (blockDim.x >> 5) * (uint32_t)(L::PLANES * PLANE_BYTES);
     unsigned long long* red = reinterpret_cast<unsigned long long*>(
-        reinterpret_cast<unsigned char*>(smem) + (rings - smem_base) + ring_bytes);              // 8 * 16 uint64
+        reinterpret_cast<unsigned char*>(smem) + stack_bytes);                                    // 8 * 16 uint64
 
     const int C = kp.chunk_bits, g = kp.gray_bits;
     const uint64_t chunk_local = (uint64_t)blockIdx.x >> kp.log2_bpc;
@@ -718,9 +750,9 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     Wk wk;
     wk.lane16 = (uint32_t)lane * 16u;
     wk.c80 = kp.c80;
-    wk.ltmask = (1u << lane) - 1u;
-    wk.ring = rings + (uint32_t)warp * (uint32_t)(L::PLANES * PLANE_BYTES);
-    wk.tail16 = 0; wk.head16 = 0;
+    const uint32_t warp_u = __reduce_min_sync(0xffffffffu, (unsigned)warp);          // the same value, known to be warp-uniform
+    wk.top = stacks + warp_u * (uint32_t)(L::PLANES * PLANE_BYTES);
+    wk.lim = wk.top + 32u * 16u;
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
     unsigned long long nz = 0;
@@ -731,7 +763,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     for (uint32_t rd = 0; rd < rounds; rd++) {
         const uint64_t q = sub * per_block + (uint64_t)rd * blockDim.x + threadIdx.x;
         wk.init_prefix(chunk_base | (q << g));
-        const uint32_t tail0 = wk.tail16;
+        wk.nzc = 0;
         // One inner block = BLK unrolled steps from inner state 0, a drain check every QUAD steps.
 #pragma unroll 1
         for (uint32_t u = 0; u < nblk; u++) {
@@ -743,7 +775,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
             });
             if (u + 1 < nblk) wk.block_end(H + (__ffs((int)(u + 1)) - 1));      // Gray order over the outer bits
         }
-        nz += (unsigned long long)((wk.tail16 - tail0) >> 4);
+        nz += (unsigned long long)wk.nzc;
     }
     wk.drain_rest();
 
@@ -774,7 +806,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
 template <int KIND, int NN>
 int launch(const KernelParams& kp, int block_threads, unsigned grid, void* stream) {
     using L = Lay<KIND, NN>;
-    const size_t smem = (size_t)RING_ALIGN + (size_t)(block_threads / 32) * L::PLANES * PLANE_BYTES
+    const size_t smem = (size_t)(block_threads / 32) * L::PLANES * PLANE_BYTES
                       + (size_t)(8 * PAIRINGS_MAX_MODULI * 2) * sizeof(uint32_t);
     cudaError_t e = cudaFuncSetAttribute(swar_kernel<KIND, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
