@@ -237,7 +237,8 @@ def run_gpu(args):
     host_rows = torch.empty((rows, m), dtype=torch.int32).pin_memory()
     host_ptr = ctypes.cast(host_rows.data_ptr(), ctypes.POINTER(ctypes.c_uint32))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-    opts = pb.LaunchOpts(variant=pb.VARIANT_AUTO)
+    opts = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=args.gray_bits, block_threads=args.block_threads,
+                         blocks_per_chunk=args.blocks_per_chunk)
 
     def barrier():
         if dist is not None:
@@ -277,7 +278,8 @@ def run_gpu(args):
 
     # ---- phi (exact non-zero fraction) from the kernel's own counter, untimed
     nzt = torch.zeros(1, dtype=torch.int64, device="cuda")
-    o2 = pb.LaunchOpts(variant=pb.VARIANT_AUTO)
+    o2 = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=args.gray_bits, block_threads=args.block_threads,
+                       blocks_per_chunk=args.blocks_per_chunk)
     o2.nonzero_terms = nzt.data_ptr()
     pb.count_pairings_ex(kind, n, C, begin, end, moduli, out.data_ptr(), stream, o2)
     torch.cuda.synchronize()
@@ -480,6 +482,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-pt", action="store_true", help="skip the approximate-counter (parallel tempering) measurement")
     ap.add_argument("--no-configs", action="store_true", help="skip the timing of the other BASELINE configs")
+    ap.add_argument("--gray-bits", type=int, default=0, help="sweep aid: pin pairings_launch_opts.gray_bits (0 = library default)")
+    ap.add_argument("--block-threads", type=int, default=0, help="sweep aid: pin block_threads (0 = library default)")
+    ap.add_argument("--blocks-per-chunk", type=int, default=0, help="sweep aid: pin blocks_per_chunk (0 = library default)")
     ap.add_argument("--profile-chunks", type=int, default=0,
                     help="profiling aid: only the first N chunks per step (short launches for ncu); the line is marked, not a bench value")
     args = ap.parse_args()

@@ -162,7 +162,14 @@ struct Lay {
     static constexpr int SIGN_SLOT = slot_of_d(NN);     // exists for both kinds (Skolem k = n, Langford k = n-1)
     static_assert(SIGN_SLOT >= 0, "distance n");
     static constexpr int EW = NR;                       // ring entry words (the packed sums)
-    static constexpr int PLANES = (EW + 3) / 4;         // 16-byte planes per entry
+    static constexpr int PLANES = (EW + 3) / 4;         // planes per entry: plane 0 holds words 0..3 at a 16-byte stride
+    // Plane 1 (words 4..) of a 5- or 6-word entry is COMPACT: 4 or 8 bytes per entry at that stride, so that the
+    // 32-/64-bit accesses of a warp fall into distinct banks (at a 16-byte stride they are 4-/2-way conflicts —
+    // measured: the shared-memory pipe, not the issue port, bounded v11).  Its address is (slot >> P1SHIFT) + k1.
+    static constexpr bool COMPACT1 = (EW == 5);        // EW == 6: measured slower (sparse 64-bit stores hardly conflict; the extra address costs an issue slot per step)
+    static constexpr int P1SHIFT = EW == 5 ? 2 : 1;
+    static constexpr int STACK_BYTES = COMPACT1 ? SCAP * 16 + SCAP * 4 * (EW - 4) : PLANES * SCAP * 16;   // per warp
+    static_assert(STACK_BYTES % 16 == 0, "stacks stay 16-byte aligned");
     static constexpr uint32_t PAD = 0x40;               // value of unused slots (never reads as zero)
 };
 
@@ -391,9 +398,21 @@ __device__ __forceinline__ void sts_v1_clr(uint32_t addr, uint32_t a, uint32_t w
                  :: "r"(addr), "r"(a), "r"(word), "r"(bit) : "memory");
 }
 // slot += 16 iff (word & bit) == 0 — the same predicate as the stores of that step
+#ifndef PAIRINGS_SLOT_VARIANT
+#define PAIRINGS_SLOT_VARIANT 0
+#endif
+#ifndef PAIRINGS_TOP_VARIANT
+#define PAIRINGS_TOP_VARIANT 1
+#endif
 __device__ __forceinline__ void add16_clr(uint32_t& slot, uint32_t word, uint32_t bit) {
     asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.eq.u32 p, t, 0;\n\t@p add.u32 %0, %0, 16;\n\t}"
                  : "+r"(slot) : "r"(word), "r"(bit));
+}
+// slot + 16 iff bit S of word is clear, as plain arithmetic (the result can live in another register than slot)
+template <int S>
+__device__ __forceinline__ uint32_t next_slot(uint32_t slot, uint32_t word) {
+    const uint32_t t = (word & (1u << S)) ^ (1u << S);
+    if constexpr (S >= 4) return slot + (t >> (S - 4)); else return slot + (t << (4 - S));
 }
 // one Kogge-Stone step of an inclusive scan over the lanes, two words at a time (byte fields that cannot overflow)
 template <int D>
@@ -402,6 +421,12 @@ __device__ __forceinline__ void scan_up2(uint32_t& a, uint32_t& b) {
                  "shfl.sync.up.b32 t|p, %0, %2, 0, 0xffffffff;\n\t"
                  "shfl.sync.up.b32 u, %1, %2, 0, 0xffffffff;\n\t"
                  "@p add.u32 %0, %0, t;\n\t@p add.u32 %1, %1, u;\n\t}" : "+r"(a), "+r"(b) : "n"(D));
+}
+__device__ __forceinline__ void lds_v2(uint32_t addr, uint32_t& a, uint32_t& b) {
+    asm volatile("ld.shared.v2.u32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "r"(addr) : "memory");
+}
+__device__ __forceinline__ void lds_v1(uint32_t addr, uint32_t& a) {
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(a) : "r"(addr) : "memory");
 }
 __device__ __forceinline__ void lds_v4(uint32_t addr, uint32_t& a, uint32_t& b, uint32_t& c, uint32_t& d) {
     asm volatile("ld.shared.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(a), "=r"(b), "=r"(c), "=r"(d) : "r"(addr) : "memory");
@@ -433,14 +458,20 @@ __device__ __forceinline__ long long upper64(long long v) {
 
 // One stack entry (at shared byte address `addr` in plane 0) -> signed multi-word term -> acc.
 template <int KIND, int NN>
-__device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t (&acc)[Lay<KIND, NN>::W], uint32_t c80) {
+__device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t k1, uint32_t (&acc)[Lay<KIND, NN>::W], uint32_t c80) {
     using L = Lay<KIND, NN>;
     constexpr int NR = L::NR, G = L::G, W = L::W, PL = L::PLANES;
     uint32_t e[4 * PL];
-    static_for<0, PL>([&](auto pc) {
-        PAIRINGS_IC(pl, pc);
-        lds_v4(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
-    });
+    if constexpr (L::COMPACT1) {
+        lds_v4(addr, e[0], e[1], e[2], e[3]);
+        const uint32_t a1 = (addr >> L::P1SHIFT) + k1;
+        if constexpr (L::EW == 5) lds_v1(a1, e[4]); else lds_v2(a1, e[4], e[5]);
+    } else {
+        static_for<0, PL>([&](auto pc) {
+            PAIRINGS_IC(pl, pc);
+            lds_v4(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
+        });
+    }
     uint32_t w[NR];
     static_for<0, NR>([&](auto rc) {                                              // bytes -> two's complement Q
         PAIRINGS_IC(r, rc);
@@ -547,6 +578,7 @@ struct Walker {
     // entry, in any order).  top = shared byte address (plane 0) of the first free entry, warp-uniform.
     uint32_t top;
     uint32_t lim;             // stack base + 32 entries: a full drain round is possible while top >= lim
+    uint32_t k1;              // compact plane 1: address of an entry's words 4.. = (plane-0 address >> P1SHIFT) + k1
     uint32_t lane16;          // lane * 16
     uint32_t c80;             // 0x80808080 (KernelParams::c80)
     uint32_t Vo;              // outer sign word: bit i = index bit H + i (set <-> x = -1)
@@ -555,7 +587,7 @@ struct Walker {
     // non-zero steps of quad 2j+w in the lanes below this one, byte j of tot[w] = that count over the whole warp.
     uint32_t ex[2], tot[2];
     uint32_t slot;            // this lane's next free entry of the current quad (lane-major inside a quad)
-    uint32_t nzc;             // non-zero terms pushed by the warp (warp-uniform, 32-bit: reset per prefix)
+    uint32_t nzc;             // non-zero terms pushed by this lane (32-bit: reset per prefix)
 
     // Row a4 for the whole block: OR over the even-distance slots of the table masks (see ztab above).
     __device__ __forceinline__ void zero_mask() {
@@ -592,31 +624,47 @@ struct Walker {
         // warp totals by REDUX (a byte sum is at most 128: no carry between fields): provably warp-uniform, which the
         // stack pointer and every drain loop inherit — the compiler then knows the warp stays converged
         tot[0] = __reduce_add_sync(0xffffffffu, c0); tot[1] = __reduce_add_sync(0xffffffffu, c1);
-        nzc = __dp4a(tot[0], 0x01010101u, __dp4a(tot[1], 0x01010101u, nzc));
+        nzc += (uint32_t)__popc(nzm);
     }
 
     template <int S>
     __device__ __forceinline__ void push_if_nonzero() {
         constexpr uint32_t bit = 1u << S;
+#if PAIRINGS_SLOT_VARIANT == 1
+        // the slot of the lane's next non-zero step goes to ANOTHER register, computed before the stores: an in-place
+        // add would have to wait until the (variable-latency) stores have read their address register
+        uint32_t nxt = slot;
+        if constexpr (S % QUAD != QUAD - 1) nxt = next_slot<S>(slot, ZM);
+#endif
         // entry words: Q[0..NR); plane p holds words 4p..4p+3 (predicated vector stores, no branch)
-        uint32_t e[4 * L::PLANES];
+        if constexpr (L::COMPACT1) {
+            sts_v4_clr(slot, Q[0], Q[1], Q[2], Q[3], ZM, bit);
+            const uint32_t a1 = (slot >> L::P1SHIFT) + k1;
+            if constexpr (EW == 5) sts_v1_clr(a1, Q[4], ZM, bit); else sts_v2_clr(a1, Q[4], Q[5], ZM, bit);
+        } else {
+            uint32_t e[4 * L::PLANES];
 #pragma unroll
-        for (int i = 0; i < 4 * L::PLANES; i++) e[i] = Q[i < NR ? i : 0];
-        static_for<0, L::PLANES>([&](auto pc) {
-            PAIRINGS_IC(pl, pc);
-            constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
-            if constexpr (words >= 3) sts_v4_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
-            else if constexpr (words == 2) sts_v2_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
-            else sts_v1_clr(slot + pl * PLANE_BYTES, e[4 * pl], ZM, bit);
-        });
+            for (int i = 0; i < 4 * L::PLANES; i++) e[i] = Q[i < NR ? i : 0];
+            static_for<0, L::PLANES>([&](auto pc) {
+                PAIRINGS_IC(pl, pc);
+                constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
+                if constexpr (words >= 3) sts_v4_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
+                else if constexpr (words == 2) sts_v2_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
+                else sts_v1_clr(slot + pl * PLANE_BYTES, e[4 * pl], ZM, bit);
+            });
+        }
+#if PAIRINGS_SLOT_VARIANT == 1
+        slot = nxt;
+#else
         if constexpr (S % QUAD != QUAD - 1) add16_clr(slot, ZM, bit);
+#endif
     }
 
     __device__ __forceinline__ void drain_full() {
         while (top >= lim) {                                   // warp-uniform
             top -= 32u * 16u;
             __syncwarp();
-            drain_entry<KIND, NN>(top + lane16, acc, c80);
+            drain_entry<KIND, NN>(top + lane16, k1, acc, c80);
             __syncwarp();
         }
     }
@@ -625,7 +673,7 @@ struct Walker {
         drain_full();
         const uint32_t base = lim - 32u * 16u;
         __syncwarp();
-        if (lane16 < top - base) drain_entry<KIND, NN>(base + lane16, acc, c80);
+        if (lane16 < top - base) drain_entry<KIND, NN>(base + lane16, k1, acc, c80);
         top = base;
         __syncwarp();
     }
@@ -635,13 +683,22 @@ struct Walker {
     template <int QI>
     __device__ __forceinline__ void quad() {
         constexpr uint32_t sel16 = 16u << (8 * (QI >> 1));                 // 16 * byte (QI >> 1) of word (QI & 1)
+#if PAIRINGS_TOP_VARIANT == 0
         slot = __dp4a(ex[QI & 1], sel16, top);
+#else
+        slot = __dp4a(ex[QI & 1], sel16, 0u) + top;                        // top is warp-uniform: [R + UR] addressing
+#endif
         static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
             PAIRINGS_IC(S, sc);
             push_if_nonzero<S>();
             if constexpr (S + 1 < BLK) inner_flip<zbits(S), ctz_c(S + 1)>();
         });
+#if PAIRINGS_TOP_VARIANT == 0
         top = __dp4a(tot[QI & 1], sel16, top);
+#else
+        constexpr int sh = 8 * (QI >> 1);                                  // uniform datapath: shift, mask, add
+        if constexpr (sh >= 4) top += (tot[QI & 1] >> (sh - 4)) & 0xFF0u; else top += (tot[QI & 1] << 4) & 0xFF0u;
+#endif
     }
 
     // flip of inner bit bi in inner state ZB: dQ = -x_j * C[bi] + K  (row a3; K = inner neighbours, folded)
@@ -725,16 +782,19 @@ template <int KIND, int NN>
 #ifndef PAIRINGS_SWAR_MINB
 #define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM (the ring limits it to 3 anyway): at most 85 registers; measured faster than 2 blocks without spills at n = 24
 #endif
-__global__ void __launch_bounds__(256, PAIRINGS_SWAR_MINB)
+#ifndef PAIRINGS_SWAR_MAXT
+#define PAIRINGS_SWAR_MAXT 256
+#endif
+__global__ void __launch_bounds__(PAIRINGS_SWAR_MAXT, PAIRINGS_SWAR_MINB)
 swar_kernel(const __grid_constant__ KernelParams kp) {
     using L = Lay<KIND, NN>;
     using Wk = Walker<KIND, NN>;
     constexpr int N = L::N, B = N - 1, W = L::W;
     extern __shared__ uint32_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // dynamic shared memory (16-byte aligned): [stacks: warps x PLANES x PLANE_BYTES][reduction scratch]
+    // dynamic shared memory (16-byte aligned): [stacks: warps x STACK_BYTES][reduction scratch]
     const uint32_t stacks = (uint32_t)__cvta_generic_to_shared(smem);
-    const uint32_t stack_bytes = (blockDim.x >> 5) * (uint32_t)(L::PLANES * PLANE_BYTES);
+    const uint32_t stack_bytes = (blockDim.x >> 5) * (uint32_t)L::STACK_BYTES;
     unsigned long long* red = reinterpret_cast<unsigned long long*>(
         reinterpret_cast<unsigned char*>(smem) + stack_bytes);                                    // 8 * 16 uint64
 
@@ -751,8 +811,9 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     wk.lane16 = (uint32_t)lane * 16u;
     wk.c80 = kp.c80;
     const uint32_t warp_u = __reduce_min_sync(0xffffffffu, (unsigned)warp);          // the same value, known to be warp-uniform
-    wk.top = stacks + warp_u * (uint32_t)(L::PLANES * PLANE_BYTES);
+    wk.top = stacks + warp_u * (uint32_t)L::STACK_BYTES;
     wk.lim = wk.top + 32u * 16u;
+    wk.k1 = wk.top + (uint32_t)(SCAP * 16) - (wk.top >> L::P1SHIFT);     // plane 1 starts behind plane 0
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
     unsigned long long nz = 0;
@@ -798,15 +859,14 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
         const uint32_t two_ne = montmul(1u << L::n_even(), mp.r2, mp.p, mp.pinv_neg);                  // 2^{#even} * 2^32
         vals[i] = montmul(r, two_ne, mp.p, mp.pinv_neg);
     }
-    // lane 0 of each warp carries the warp's non-zero count (tail is warp-uniform)
     __syncthreads();
-    block_reduce_write(kp, vals, lane == 0 ? nz : 0ULL, red, chunk_local);
+    block_reduce_write(kp, vals, nz, red, chunk_local);
 }
 
 template <int KIND, int NN>
 int launch(const KernelParams& kp, int block_threads, unsigned grid, void* stream) {
     using L = Lay<KIND, NN>;
-    const size_t smem = (size_t)(block_threads / 32) * L::PLANES * PLANE_BYTES
+    const size_t smem = (size_t)(block_threads / 32) * L::STACK_BYTES
                       + (size_t)(8 * PAIRINGS_MAX_MODULI * 2) * sizeof(uint32_t);
     cudaError_t e = cudaFuncSetAttribute(swar_kernel<KIND, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
