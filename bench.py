@@ -7,18 +7,24 @@ A "step" is one pass of the whole hot path over the workload: partition -> count
 Gray-code kernel over every chunk of this rank's range) -> rows D2H -> row sums -> (rank 0, after
 the exchange of the per-rank sums) CRT + exact division, checked against the paper's printed count.
 Workload at every N: Langford L(20) — 2^39 sign vectors (x_1 = +1), 2^16 prefix chunks, 6 CRT primes
-+ 1 check prime (BASELINE.json configs[3], the n = 20 point the metric is quoted on).  For N > 1 the path shards
-by chunk ranges with no data-path collective; the default (`--scaling weak`) keeps the per-GPU work fixed: every
-rank evaluates a whole L(20) pass and rank 0 checks that all ranks' residue sums agree (the paper's duplicate-run
-protocol, one copy per GPU); `--scaling strong` deals the 2^16 chunks out as contiguous ranges
-(pairings_rank_range), total work fixed.
++ 1 check prime (BASELINE.json configs[3], the n = 20 point the metric is quoted on).
+
+N > 1: the path shards by chunk ranges with no data-path collective ("split ... into several
+independent sets and simply put the result together at the end").  `--gpus N` starts the N ranks itself when it is not
+already running under torchrun (WORLD_SIZE unset): N copies of this script with RANK / LOCAL_RANK / WORLD_SIZE /
+MASTER_ADDR=127.0.0.1 / MASTER_PORT set, one GPU each, NCCL for the barrier and the exchange of the per-rank residue
+sums.  Under torchrun WORLD_SIZE must equal --gpus.  The ranks take DISJOINT chunk ranges (pairings_rank_range; total
+work fixed: "scaling": "strong"), their sums are added and L(20) is reconstructed from them.  `--scaling duplicate`
+(opt-in) is the paper's duplicate-run check (PAPER.md:99): every rank evaluates the whole pass, the copies must agree;
+its `value` counts the sign vectors ONCE.
 
 `value`   = terms/s with the rows left in HBM (CUDA events around the kernel launches of a step).
 `e2e`     = terms/s through count_pairings_host (HOST output buffer; allocation, launch, D2H copy
             and synchronise inside the timed region, wall clock).
-`roofline`= SURVEY.md §8(d) yardstick ops/term (W + phi*M, phi measured live) x terms/s against the
-            SM integer-issue peak 148 x 128 lanes x sm_max_mhz; calibration kernels measured beside it.
-`cpu_baseline` = the CPU oracle (oracle/, as it stands) on the host cores, bounded sample.
+`roofline`= SURVEY.md §8(d): `frac` on the fixed yardstick ops/term (W + phi*M, phi measured live) x terms/s
+            against the SM integer-issue peak 148 x 128 lanes x sm_max_mhz; beside it the EXECUTED thread-instructions
+            per term of the profiled kernel (profiles/ncu_metrics.json) and the issue-slot fraction they give.
+`cpu_baseline` = the CPU oracle (oracle/, as it stands) on the host cores, bounded sample, all cores and 1 core.
 """
 from __future__ import annotations
 
@@ -26,6 +32,7 @@ import argparse
 import ctypes
 import json
 import os
+import socket
 import statistics
 import subprocess
 import sys
@@ -51,6 +58,7 @@ OTHER_CONFIGS = [(1, 12, 6, 4, 100, 108144), (0, 13, 8, 4, 100, 1520280), (1, 16
                  (0, 16, 10, 6, 20, 700078384), (0, 21, 18, 7, 1, 61782464083584)]
 PT_BETAS = [0, 0.54, 1.1, 1.69, 2.33, 3, 3.73, 4.65, 5.82, 8.1, 16, 32]     # PAPER.md:329-341 (Table 6, column beta)
 SM_COUNT, LANES_PER_SM_CLK = 148, 128
+NCU_METRICS = os.path.join(ROOT, "profiles", "ncu_metrics.json")
 
 
 def yardstick_ops(kind: int, n: int, n_moduli: int, phi: float):
@@ -65,6 +73,37 @@ def yardstick_ops(kind: int, n: int, n_moduli: int, phi: float):
     W = 3 * n + 3
     M = (n - G) + n_moduli * (5 * (G - 1) + 3)
     return W + phi * M, dict(W=W, M=M, G=G, phi=phi)
+
+
+def ncu_metrics(kind: int, n: int):
+    """The executed-instruction record of the profiled kernel instance (written by
+    `python -m paper_1507_00315_b200.ncu_summary` from an `ncu --set full` capture), or None."""
+    try:
+        with open(NCU_METRICS) as f:
+            return json.load(f)["instances"].get("%s%d" % (KIND_NAME[kind], n))
+    except (OSError, ValueError, KeyError):
+        return None
+
+
+def roofline_object(kind, n, n_moduli, phi, terms_per_launch, kernel_s, peak_mhz):
+    """SURVEY §8(d)'s three numbers: terms/s (in the line), the model fraction on the fixed yardstick (`frac`), and
+    the executed thread-instructions per term with the issue-slot fraction they give."""
+    ops, ys = yardstick_ops(kind, n, n_moduli, phi)
+    peak = SM_COUNT * LANES_PER_SM_CLK * peak_mhz * 1e6
+    rate = terms_per_launch / kernel_s
+    achieved = ops * rate
+    r = dict(bound="alu", achieved=achieved / 1e12, peak=peak / 1e12, unit="Tinstr/s", frac=achieved / peak, traffic=None,
+             peak_source="formula: 148 SM x 128 lanes/clk x %.0f MHz (clocks.max.sm); MEASURED_PEAKS.json has no integer figure" % peak_mhz,
+             ops_per_term=ops, yardstick=ys, kernel_ms=kernel_s * 1e3, terms_per_launch=terms_per_launch,
+             frac_note="frac is on the fixed yardstick of SURVEY.md §8(d) (3n+3 scalar ops per step, per-term Montgomery chains); this "
+                       "kernel needs fewer instructions than that (packed sums, table-driven zero test, residues once per thread), so "
+                       "frac > 1; issue_frac = executed instructions x terms/s / peak is the utilisation figure")
+    m = ncu_metrics(kind, n)
+    if m:
+        r.update(executed_instr_per_term=m["instr_per_term"], issue_frac=m["instr_per_term"] * rate / peak,
+                 issue_active_pct=m["issue_active_pct"], ncu_source=m.get("source"), ncu_commit=m.get("commit"),
+                 traffic=m.get("dram_bytes_per_launch"))
+    return r
 
 
 def host_threads() -> int:
@@ -103,7 +142,7 @@ def oracle_sample(kind, n, sample_bits, chunks, threads):
     return terms, dt
 
 
-def cpu_baseline(kind, n, target_seconds=15.0):
+def cpu_baseline(kind, n, target_seconds=12.0):
     from paper_1507_00315_b200 import seeds
     threads = host_threads()
     sample_bits = 2 * n - 1 - 17                       # 2^17 terms per oracle chunk
@@ -113,9 +152,13 @@ def cpu_baseline(kind, n, target_seconds=15.0):
     count = int(max(threads, min(4096, target_seconds * rate / (1 << 17))))
     chunks = seeds.sample_chunks(sample_bits, count, salt=11)
     terms, dt = oracle_sample(kind, n, sample_bits, chunks, threads)
-    return dict(value=terms / dt, unit="terms/s", cores=threads, kind="oracle",
+    # one core ("report terms/s for 1 core and all cores"): ~4 s of the same kind of chunks
+    one = seeds.sample_chunks(sample_bits, int(max(2, min(512, 4.0 * rate / threads / (1 << 17)))), salt=13)
+    terms1, dt1 = oracle_sample(kind, n, sample_bits, one, 1)
+    return dict(value=terms / dt, unit="terms/s", cores=threads, kind="oracle", value_1core=terms1 / dt1,
                 sample="%d seeded chunks of 2^17 sign vectors of %s(%d) (2^%d-chunk partition of the x_1=+1 half), "
-                       "%.1f s on %d threads" % (len(chunks), KIND_NAME[kind], n, sample_bits, dt, threads))
+                       "%.1f s on %d threads; 1 core: %d such chunks, %.1f s" %
+                       (len(chunks), KIND_NAME[kind], n, sample_bits, dt, threads, len(one), dt1))
 
 
 def run_reference(args):
@@ -139,7 +182,7 @@ def run_reference(args):
     sample = "%d seeded chunks of 2^17 sign vectors of L(20) per step on %d threads" % (per_step, threads)
     line = dict(impl="reference", metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s",
                 n_gpus=args.gpus, steps=steps, warmup=warm, ms_per_step=1e3 * t_total / steps,
-                higher_is_better=True, scaling=args.scaling, vs_baseline=None, dtype="int32", data="synthetic",
+                higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
                 config=dict(workload=WORKLOAD, kind="langford", n=n, chunk_bits=WL["chunk_bits"], n_moduli=WL["n_moduli"],
                             sample="each step is a bounded sample of the workload: " + sample),
                 cpu_baseline=dict(value=value, unit="terms/s", cores=threads, kind="oracle", sample=sample),
@@ -183,7 +226,7 @@ class ClockSampler:
         if self.proc is None:
             return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
         time.sleep(0.25)
-        sm, mx, reasons = [], None, set()
+        sm, mx, power, reasons = [], None, [], set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for t, ln in self.lines:
             if t < t0 or t > t1 + 0.3:
@@ -192,12 +235,33 @@ class ClockSampler:
             try:
                 sm.append(float(f[0]))
                 mx = float(f[1])
+                power.append(float(f[2]))
             except (ValueError, IndexError):
                 continue
             for name, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
-        return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=mx, samples=len(sm), reasons=sorted(reasons))
+        return dict(sm_mhz=statistics.median(sm) if sm else None, sm_max_mhz=mx, samples=len(sm),
+                    power_w_max=max(power) if power else None, reasons=sorted(reasons))
+
+
+_probe_lib = None
+
+
+def issue_probe(mode, blocks, threads, iters, out_dev_ptr, stream):
+    """Enqueues a calibration kernel of libpairings_probe.so (bench-side, not in the product library); returns the
+    number of thread-instructions it executes."""
+    global _probe_lib
+    if _probe_lib is None:
+        from paper_1507_00315_b200 import build as pbuild
+        _probe_lib = ctypes.CDLL(pbuild.build_probe())
+        _probe_lib.pairings_issue_probe.restype = ctypes.c_int
+        _probe_lib.pairings_issue_probe.argtypes = [ctypes.c_int] * 4 + [ctypes.c_void_p, ctypes.c_void_p, ctypes.POINTER(ctypes.c_uint64)]
+    cnt = ctypes.c_uint64(0)
+    rc = _probe_lib.pairings_issue_probe(mode, blocks, threads, iters, ctypes.c_void_p(out_dev_ptr), ctypes.c_void_p(stream), ctypes.byref(cnt))
+    if rc:
+        raise RuntimeError("pairings_issue_probe failed: %d" % rc)
+    return int(cnt.value)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -215,8 +279,13 @@ def run_gpu(args):
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus:
+        raise SystemExit("bench.py: --gpus %d but WORLD_SIZE=%d (start it as `python bench.py --gpus N`, which spawns the ranks "
+                         "itself, or under torchrun with --nproc-per-node equal to --gpus)" % (args.gpus, world))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (there is no CPU fallback); use --impl reference for the oracle")
+    if local >= torch.cuda.device_count():
+        raise SystemExit("bench.py: rank %d needs cuda:%d but only %d device(s) are visible" % (rank, local, torch.cuda.device_count()))
     torch.cuda.set_device(local)
     dist = None
     if world > 1:
@@ -225,20 +294,29 @@ def run_gpu(args):
 
     kind, n, C, m = WL["kind"], WL["n"], WL["chunk_bits"], WL["n_moduli"]
     moduli = pb.pairings_default_moduli(m)
-    weak = args.scaling == "weak"
-    begin, end = (0, 1 << C) if weak else pb.pairings_rank_range(C, rank, world)
+    duplicate = args.scaling == "duplicate"
+    begin, end = (0, 1 << C) if duplicate else pb.pairings_rank_range(C, rank, world)
     if args.profile_chunks:                      # short launches for ncu captures; not a bench value
         end = min(end, begin + args.profile_chunks)
     rows = end - begin
     terms_rank = rows << (2 * n - 1 - C)
-    terms_job = terms_rank * world if (weak or args.profile_chunks) else (1 << (2 * n - 1))
+    # sign vectors of the JOB, each counted once (duplicate mode: N copies of the same pass are one pass)
+    terms_job = terms_rank * (1 if duplicate else world) if args.profile_chunks else (1 << (2 * n - 1))
     stream = torch.cuda.current_stream().cuda_stream
     out = torch.empty((rows, m), dtype=torch.int32, device="cuda")
     host_rows = torch.empty((rows, m), dtype=torch.int32).pin_memory()
     host_ptr = ctypes.cast(host_rows.data_ptr(), ctypes.POINTER(ctypes.c_uint32))
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
-    opts = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=args.gray_bits, block_threads=args.block_threads,
-                         blocks_per_chunk=args.blocks_per_chunk)
+
+    def launch_opts(nonzero_ptr=None):
+        o = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=args.gray_bits, block_threads=args.block_threads,
+                          blocks_per_chunk=args.blocks_per_chunk)
+        if nonzero_ptr is not None:
+            o.nonzero_terms = nonzero_ptr
+        return o
+
+    opts = launch_opts()
+    geometry = pb.pairings_query_geometry(kind, n, C, rows, opts)
 
     def barrier():
         if dist is not None:
@@ -256,7 +334,7 @@ def run_gpu(args):
             t = torch.tensor(total, dtype=torch.int64, device="cuda")
             gathered = [torch.zeros_like(t) for _ in range(world)]
             dist.all_gather(gathered, t)
-            if weak:                                     # every rank counted everything: the copies must agree
+            if duplicate:                                # every rank counted everything: the copies must agree
                 assert all(g.tolist() == total for g in gathered), "ranks disagree (PAPER.md:99 duplicate-run check)"
             else:
                 total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
@@ -269,7 +347,8 @@ def run_gpu(args):
     sampler.start()
 
     # ---- warm-up (>= 3), correctness of the warmed-up path
-    for _ in range(max(args.warmup, 3) if args.warmup >= 0 else 3):
+    warm = max(args.warmup, 3)
+    for _ in range(warm):
         step_device()
         flush.fill_(1)
     torch.cuda.synchronize()
@@ -278,10 +357,7 @@ def run_gpu(args):
 
     # ---- phi (exact non-zero fraction) from the kernel's own counter, untimed
     nzt = torch.zeros(1, dtype=torch.int64, device="cuda")
-    o2 = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=args.gray_bits, block_threads=args.block_threads,
-                       blocks_per_chunk=args.blocks_per_chunk)
-    o2.nonzero_terms = nzt.data_ptr()
-    pb.count_pairings_ex(kind, n, C, begin, end, moduli, out.data_ptr(), stream, o2)
+    pb.count_pairings_ex(kind, n, C, begin, end, moduli, out.data_ptr(), stream, launch_opts(nzt.data_ptr()))
     torch.cuda.synchronize()
     phi = float(nzt.item()) / terms_rank
 
@@ -300,13 +376,13 @@ def run_gpu(args):
     t_end = time.perf_counter()
     clocks = sampler.window(t_begin, t_end)
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
+    rank_kernel_s = dev_ms * 1e-3 / args.steps            # this rank's kernel
     if dist is not None:
         t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         dev_ms = float(t.item())
-    launches = args.steps                       # one kernel launch per step and rank (grid = chunks of the rank)
+    launches = (warm + 1 + args.steps) * world  # one kernel launch per pass and rank (grid = chunks of the rank)
     value = terms_job * args.steps / (dev_ms * 1e-3)
-    kernel_s = dev_ms * 1e-3 / args.steps
 
     # ---- e2e: the public host-buffer call, wall clock, copies + allocation inside
     for _ in range(2):
@@ -319,16 +395,17 @@ def run_gpu(args):
     barrier()
     e2e_s = time.perf_counter() - t0
     clocks_e2e = sampler.window(t0, t0 + e2e_s)
-    sampler.close()
     if dist is not None:
         t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_s = float(t.item())
     e2e_value = terms_job * args.steps / e2e_s
+    launches += (2 + args.steps) * world
 
+    extras = rank == 0 and world == 1 and not args.profile_chunks      # the single-GPU side measurements
     # ---- whole count with symmetry 3 (Lemma 2.4, §8(f) NEXT #1): half the chunks, doubled; wall clock, rank 0
     lemma24 = None
-    if rank == 0 and world == 1 and not args.profile_chunks:
+    if extras:
         t0 = time.perf_counter()
         tot, done, needed = pb.pairings_run_ex(kind, n, C, moduli, 1 << C, None, 0, stream, opts, pb.RUN_LEMMA24)
         dt = time.perf_counter() - t0
@@ -336,18 +413,13 @@ def run_gpu(args):
         assert S == L20_IDENTIFIED and done == needed == 1 << (C - 1)
         lemma24 = dict(seconds=dt, chunks_evaluated=needed, terms_evaluated=needed << (2 * n - 1 - C),
                        note="pairings_run_ex(PAIRINGS_RUN_LEMMA24): x_2 = +1 half of the chunks, doubled; same count")
+        launches += 1
 
     line = None
     if rank == 0:
-        ops, ys = yardstick_ops(kind, n, m, phi)
         peak_mhz = clocks.get("sm_max_mhz") or 1965.0
         peak = SM_COUNT * LANES_PER_SM_CLK * peak_mhz * 1e6
-        achieved = ops * (terms_rank / kernel_s)           # this rank's kernel: algorithmic thread-instr/s
-        roofline = dict(bound="alu", achieved=achieved / 1e12, peak=peak / 1e12, unit="Tinstr/s",
-                        frac=achieved / peak, traffic=None,
-                        peak_source="formula: 148 SM x 128 lanes/clk x %.0f MHz (clocks.max.sm); MEASURED_PEAKS.json has no integer figure" % peak_mhz,
-                        ops_per_term=ops, yardstick=ys,
-                        kernel_ms=kernel_s * 1e3, terms_per_launch=terms_rank)
+        roofline = roofline_object(kind, n, m, phi, terms_rank, rank_kernel_s, peak_mhz)
         # calibration kernels: measured thread-instr/s per instruction class
         cal = {}
         scratch = torch.zeros(4, dtype=torch.int32, device="cuda")
@@ -356,47 +428,63 @@ def run_gpu(args):
             for rep in range(3):
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()
-                cnt = pb.pairings_issue_probe(mode, SM_COUNT * 8, 256, 4096, scratch.data_ptr(), stream)
+                cnt = issue_probe(mode, SM_COUNT * 8, 256, 4096, scratch.data_ptr(), stream)
                 e1.record()
                 torch.cuda.synchronize()
                 best = max(best, cnt / (e0.elapsed_time(e1) * 1e-3))
             cal[name] = best / 1e12
         roofline["calibration_Tinstr_per_s"] = cal
-        roofline["frac_of_best_calibration"] = achieved / 1e12 / max(cal.values())
+        roofline["frac_of_best_calibration"] = roofline["achieved"] / max(cal.values())
+        if "issue_frac" in roofline:
+            roofline["issue_frac_of_best_calibration"] = roofline["issue_frac"] * roofline["peak"] / max(cal.values())
 
-        # secondary point of the metric: S(24) on the seeded 1/64 subset
+        # secondary point of the metric: S(24) on the seeded 1/64 subset (BASELINE.json configs[4])
         n24 = None
-        if not args.no_n24:
+        if not args.no_n24 and world == 1:
             k2, n2, C2, m2 = WL24["kind"], WL24["n"], WL24["chunk_bits"], WL24["n_moduli"]
             mod2 = pb.pairings_default_moduli(m2)
-            starts = seeds.sample_range_starts(C2, max(1, int(WL24["runs"] * args.n24_fraction)), WL24["run_len"])
+            runs = max(1, int(round(WL24["runs"] * args.n24_fraction)))
+            starts = seeds.sample_range_starts(C2, runs, WL24["run_len"])
             out2 = torch.empty((WL24["run_len"], m2), dtype=torch.int32, device="cuda")
-            pb.count_pairings_ex(k2, n2, C2, starts[0], starts[0] + WL24["run_len"], mod2, out2.data_ptr(), stream, opts)
+            nz24 = torch.zeros(1, dtype=torch.int64, device="cuda")
+            o24 = launch_opts(nz24.data_ptr())
+            # untimed: every run once with the non-zero counter = warm-up launches (>= 2) and the exact phi of the subset
+            warm24 = starts if len(starts) >= 2 else starts * 2
+            for s0 in warm24:
+                pb.count_pairings_ex(k2, n2, C2, s0, s0 + WL24["run_len"], mod2, out2.data_ptr(), stream, o24)
             torch.cuda.synchronize()
+            terms24 = len(starts) * WL24["run_len"] << (2 * n2 - 1 - C2)
+            phi24 = float(nz24.item()) / (terms24 * len(warm24) // len(starts))
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
             for s0 in starts:
                 pb.count_pairings_ex(k2, n2, C2, s0, s0 + WL24["run_len"], mod2, out2.data_ptr(), stream, opts)
             e1.record()
             torch.cuda.synchronize()
+            t1 = time.perf_counter()
             t24 = e0.elapsed_time(e1) * 1e-3
-            terms24 = len(starts) * WL24["run_len"] << (2 * n2 - 1 - C2)
-            n24 = dict(workload="S(24): %d seeded runs of %d contiguous chunks of the 2^20-chunk partition, 8+1 primes" % (len(starts), WL24["run_len"]),
-                       terms=terms24, seconds=t24, value=terms24 / t24, unit="terms/s",
-                       projected_full_run_s=(1 << 47) / (terms24 / t24))
+            launches += len(warm24) + len(starts)
+            n24 = dict(workload="S(24): %d seeded runs of %d contiguous chunks of the 2^20-chunk partition (= 1/%d of the chunks), 8+1 primes"
+                                % (len(starts), WL24["run_len"], (1 << C2) // (len(starts) * WL24["run_len"])),
+                       terms=terms24, seconds=t24, value=terms24 / t24, unit="terms/s", launches=len(starts), warmup_launches=len(warm24),
+                       geometry=dict(zip(("variant", "gray_bits", "block_threads", "blocks_per_chunk"),
+                                         pb.pairings_query_geometry(k2, n2, C2, WL24["run_len"], opts))),
+                       clocks=sampler.window(t0, t1), projected_full_run_s=(1 << 47) / (terms24 / t24),
+                       roofline=roofline_object(k2, n2, m2, phi24, terms24 // len(starts), t24 / len(starts), peak_mhz))
 
         # the other BASELINE.json configs (parity-test cases; timed here for SURVEY §8(d)'s per-config table)
         other = None
-        if not args.no_configs and world == 1 and not args.profile_chunks:
+        if not args.no_configs and extras:
             other = []
             for (k2, n2, C2, m2, reps, want) in OTHER_CONFIGS:
                 mod2 = pb.pairings_default_moduli(m2)
                 rows2 = 1 << C2
                 out2 = torch.empty((rows2, m2), dtype=torch.int32, device="cuda")
                 nz2 = torch.zeros(1, dtype=torch.int64, device="cuda")
-                o3 = pb.LaunchOpts(variant=pb.VARIANT_AUTO)
-                o3.nonzero_terms = nz2.data_ptr()
-                pb.count_pairings_ex(k2, n2, C2, 0, rows2, mod2, out2.data_ptr(), stream, o3)    # warm-up + phi
+                pb.count_pairings_ex(k2, n2, C2, 0, rows2, mod2, out2.data_ptr(), stream, launch_opts(nz2.data_ptr()))    # warm-up + phi
                 torch.cuda.synchronize()
                 flat2 = (ctypes.c_uint32 * (rows2 * m2)).from_buffer_copy(out2.cpu().numpy().tobytes())
                 D2, S2 = pb.pairings_reconstruct(k2, n2, mod2, pb.pairings_sum_rows(flat2, mod2))
@@ -408,16 +496,39 @@ def run_gpu(args):
                 e1.record()
                 torch.cuda.synchronize()
                 sec = e0.elapsed_time(e1) * 1e-3 / reps
+                launches += reps + 1
                 terms2 = 1 << (2 * n2 - 1)
                 phi2 = float(nz2.item()) / terms2
                 ops2, ys2 = yardstick_ops(k2, n2, m2, phi2)
-                other.append(dict(config="%s(%d)" % (KIND_NAME[k2], n2), chunk_bits=C2, n_moduli=m2, launches_timed=reps,
-                                  seconds_per_count=sec, value=terms2 / sec, unit="terms/s", phi=phi2, ops_per_term=ops2,
-                                  roofline_frac=ops2 * terms2 / sec / peak, identified=S2))
+                entry = dict(config="%s(%d)" % (KIND_NAME[k2], n2), chunk_bits=C2, n_moduli=m2, launches_timed=reps,
+                             seconds_per_count=sec, value=terms2 / sec, unit="terms/s", phi=phi2, ops_per_term=ops2,
+                             roofline_frac=ops2 * terms2 / sec / peak, identified=S2,
+                             geometry=dict(zip(("variant", "gray_bits", "block_threads", "blocks_per_chunk"),
+                                               pb.pairings_query_geometry(k2, n2, C2, rows2, opts))))
+                if reps >= 20:
+                    # launch-bound configs: the same `reps` launches replayed as ONE CUDA graph (no host launch gaps)
+                    side = torch.cuda.Stream()
+                    g = torch.cuda.CUDAGraph()
+                    with torch.cuda.stream(side):
+                        with torch.cuda.graph(g, stream=side):
+                            for _ in range(reps):
+                                pb.count_pairings_ex(k2, n2, C2, 0, rows2, mod2, out2.data_ptr(), side.cuda_stream, opts)
+                        g.replay()
+                        side.synchronize()
+                        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                        e0.record(side)
+                        g.replay()
+                        e1.record(side)
+                        side.synchronize()
+                    entry["seconds_per_count_cuda_graph"] = e0.elapsed_time(e1) * 1e-3 / reps
+                    launches += 2 * reps
+                    flat2 = (ctypes.c_uint32 * (rows2 * m2)).from_buffer_copy(out2.cpu().numpy().tobytes())
+                    assert pb.pairings_reconstruct(k2, n2, mod2, pb.pairings_sum_rows(flat2, mod2))[1] == want
+                other.append(entry)
 
         # second workload: the approximate counter, S(12) with the ladder of Table 6
         ptres = None
-        if not args.no_pt and world == 1 and not args.profile_chunks:
+        if not args.no_pt and extras:
             import math
             R, T, burn = 1 << 17, 1 << 11, 0                      # throughput run (too short per replica for an estimate)
             Mlev = len(PT_BETAS)
@@ -438,35 +549,96 @@ def run_gpu(args):
             pb.pairings_pt_run(0, 12, PT_BETAS, 0, 1 << 12, 1 << 15, 1 << 14, 150700315, h.data_ptr(), mv.data_ptr(), sw.data_ptr(), stream)
             torch.cuda.synchronize()
             est_s = time.perf_counter() - t0
+            launches += 3
             ratios, logz = pb.pairings_pt_estimate(0, 12, PT_BETAS, h.cpu().tolist())
             est = math.exp(logz) / 2
+            moves_s = R * T * Mlev / sec
             ptres = dict(workload="approximate count of S(12), 12 levels (Table 6 ladder, PAPER.md:327-342)",
-                         replicas=R, iterations=T, seconds=sec, metropolis_moves_per_s=R * T * Mlev / sec,
+                         replicas=R, iterations=T, seconds=sec, metropolis_moves_per_s=moves_s,
+                         cpu_oracle=pt_cpu_baseline(),
                          estimate=dict(replicas=1 << 12, iterations=1 << 15, burn_in=1 << 14, seconds=est_s,
                                        s12_estimate=est, exact=227968, rel_error=est / 227968 - 1))
+            if ptres["cpu_oracle"]:
+                ptres["gpu_over_cpu_oracle"] = moves_s / ptres["cpu_oracle"]["value"]
 
-        cpu = cpu_baseline(kind, n) if not args.no_cpu else None
+        cpu = cpu_baseline(kind, n) if not args.no_cpu and not args.profile_chunks else None
+        par = ("every rank the whole pass x%d, residue sums cross-checked (PAPER.md:99); each sign vector counted once" if duplicate
+               else "disjoint chunk ranges x%d (pairings_rank_range), per-rank residue sums added, no data-path collective") % world
         line = dict(metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s", n_gpus=world,
-                    steps=args.steps, warmup=max(args.warmup, 3), ms_per_step=dev_ms / args.steps,
-                    higher_is_better=True, scaling=args.scaling, vs_baseline=None, dtype="int32", data="synthetic",
+                    steps=args.steps, warmup=warm, ms_per_step=dev_ms / args.steps,
+                    higher_is_better=True, scaling="weak" if duplicate else "strong", vs_baseline=None, dtype="int32", data="synthetic",
                     config=dict(workload=WORKLOAD,
-                                kind="langford", n=n, chunk_bits=C, n_moduli=m, parallelism=("one full pass per GPU x%d, residue sums cross-checked" if weak else "disjoint chunk ranges x%d") % world,
+                                kind="langford", n=n, chunk_bits=C, n_moduli=m, parallelism=par, duplicate_run=duplicate,
+                                launcher="self-spawned ranks" if os.environ.get("PAIRINGS_BENCH_SPAWNED") else ("torchrun" if world > 1 else "single process"),
+                                geometry=dict(zip(("variant", "gray_bits", "block_threads", "blocks_per_chunk"), geometry)),
                                 sm_count=torch.cuda.get_device_properties(local).multi_processor_count,
-                                l2="flushed between steps (256 MiB fill); the kernel reads no global memory",
+                                l2="flushed between steps (256 MiB fill); the kernel reads no global memory but its 24 KB zero-step tables",
                                 result_check="L(20) = 2,636,337,861,200 reconstructed every run (PAPER.md:380)",
                                 library=pb.pairings_build_info()),
                     clocks=clocks,
-                    e2e=dict(value=e2e_value, unit="terms/s", h2d_bytes_per_step=4 * m + 8 * 5,
+                    e2e=dict(value=e2e_value, unit="terms/s", h2d_bytes_per_step=(4 * m + 8 * 5) * world,
                              d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps,
                              clocks=clocks_e2e),
                     profile_only=bool(args.profile_chunks),
                     gpu_launches=launches, roofline=roofline, cpu_baseline=cpu, n24=n24, lemma24=lemma24, other_configs=other, pt=ptres,
                     paper_context="paper's Kepler GPU: S(20) in 4.08 min ~ 1.1e9 terms/s (PAPER.md:397; other hardware, context only)")
+    sampler.close()
     if dist is not None:
         dist.barrier()
         dist.destroy_process_group()
     if line is not None:
         print(json.dumps(line))
+
+
+def pt_cpu_baseline():
+    """The PT oracle (oracle/pt_oracle.cpp, as it stands) on the host cores: Metropolis moves/s for the same ladder."""
+    try:
+        from oracle import pt
+        pt.build()
+    except Exception:                                   # no compiler on the box: report nothing rather than fail the bench
+        return None
+    threads = host_threads()
+    reps, its = 8, 1 << 12
+    res = [None] * threads
+
+    def work(t):
+        res[t] = pt.run(0, 12, PT_BETAS, reps, its, 1000 + t, 0)
+
+    t0 = time.perf_counter()
+    ts = [threading.Thread(target=work, args=(t,)) for t in range(threads)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+    dt = time.perf_counter() - t0
+    moves = threads * reps * its * len(PT_BETAS)
+    return dict(value=moves / dt, unit="metropolis moves/s", cores=threads, kind="oracle",
+                sample="%d replicas x %d iterations x %d levels per thread, %.1f s on %d threads" % (reps, its, len(PT_BETAS), dt, threads))
+
+
+# ------------------------------------------------------------------------------------------------
+# launcher: --gpus N starts its own ranks
+# ------------------------------------------------------------------------------------------------
+def _free_port():
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    p = s.getsockname()[1]
+    s.close()
+    return p
+
+
+def spawn_ranks(n: int) -> int:
+    """Starts n copies of this command line, one rank each (rank r -> cuda:r), and waits for them.  Rank 0's stdout is
+    this process's stdout (the JSON line); NCCL's own logging is left as the environment has it."""
+    port = os.environ.get("MASTER_PORT") or str(_free_port())
+    procs = []
+    for r in range(n):
+        env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), MASTER_ADDR="127.0.0.1", MASTER_PORT=port,
+                   PAIRINGS_BENCH_SPAWNED="1")
+        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env,
+                                      stdout=None if r == 0 else subprocess.DEVNULL))
+    rc = 0
+    for p in procs:
+        rc = max(rc, abs(p.wait()))
+    return rc
 
 
 def main():
@@ -475,10 +647,12 @@ def main():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--spawn", action="store_true", help="start the rank processes even for --gpus 1 (tests the launcher on one GPU)")
     ap.add_argument("--no-n24", action="store_true", help="skip the secondary S(24) subset measurement")
-    ap.add_argument("--n24-fraction", type=float, default=0.125, help="fraction of the 16 seeded S(24) runs (1024 chunks each) to time")
-    ap.add_argument("--scaling", default="weak", choices=["weak", "strong"],
-                    help="N > 1: weak = every rank a whole pass (cross-checked), strong = disjoint chunk ranges")
+    ap.add_argument("--n24-fraction", type=float, default=1.0,
+                    help="fraction of the 16 seeded S(24) runs (1024 chunks each = 1/64 of the chunks, BASELINE.json configs[4]) to time")
+    ap.add_argument("--scaling", default="strong", choices=["strong", "duplicate"],
+                    help="N > 1: strong = disjoint chunk ranges (default); duplicate = every rank the whole pass, cross-checked (PAPER.md:99)")
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-pt", action="store_true", help="skip the approximate-counter (parallel tempering) measurement")
     ap.add_argument("--no-configs", action="store_true", help="skip the timing of the other BASELINE configs")
@@ -488,6 +662,10 @@ def main():
     ap.add_argument("--profile-chunks", type=int, default=0,
                     help="profiling aid: only the first N chunks per step (short launches for ncu); the line is marked, not a bench value")
     args = ap.parse_args()
+    if args.gpus < 1:
+        ap.error("--gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and (args.gpus > 1 or args.spawn):
+        sys.exit(spawn_ranks(args.gpus))
     if args.impl == "reference":
         run_reference(args)
     else:

@@ -168,13 +168,38 @@ int pairings_sum_rows(const uint32_t* rows, uint64_t n_rows,
  * pairings_journal_append creates the file (with header) if absent and refuses (PAIRINGS_EJOURNAL)
  * a file written for other parameters.  pairings_journal_load returns the number of recorded
  * ranges (writing up to cap_ranges (begin,end) pairs) and the sum of their rows in total_out;
- * a missing file is 0 ranges.  Truncated last lines (a crash mid-write) are ignored. */
+ * a missing file is 0 ranges.  A truncated last line (a crash mid-write: bytes behind the last newline) is ignored
+ * by load and cut off by the next append; a line with missing, non-numeric or surplus tokens, a range outside
+ * [0, 2^chunk_bits) or two overlapping ranges make the file PAIRINGS_EJOURNAL.  Every append is fsync-ed. */
 int pairings_journal_append(const char* path, int kind, int n, int chunk_bits,
                             const uint32_t* moduli, int n_moduli,
                             uint64_t chunk_begin, uint64_t chunk_end, const uint32_t* row_sum);
 int64_t pairings_journal_load(const char* path, int kind, int n, int chunk_bits,
                               const uint32_t* moduli, int n_moduli,
                               uint64_t* out_ranges, int64_t cap_ranges, uint32_t* total_out);
+
+/* Puts the journals of several jobs together ("split ... into several independent sets and simply put
+ * the result together at the end"; 4 / 64 / 256 / 1024 GPU jobs): every file of paths[0..n_paths) must
+ * exist and carry the header of (kind, n, chunk_bits, moduli); their ranges must not overlap each other (a chunk
+ * counted twice: PAIRINGS_EJOURNAL).  total_out (HOST, n_moduli) = sum of all rows; *chunks_covered_out (may be NULL) =
+ * number of chunks they cover (the job is complete when it equals the number of chunks evaluated in that mode);
+ * out_path (may be NULL) receives one merged journal, ranges ascending, written and fsync-ed.  Returns the number of
+ * ranges or a negative code.  Host only. */
+int64_t pairings_journal_merge(const char* const* paths, int n_paths, const char* out_path,
+                               int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                               uint32_t* total_out, uint64_t* chunks_covered_out);
+
+/* The duplicate-run protocol against silent GPU errors ("every GPU job was ran twice on separate GPUs.
+ * The two results were then matched, if there was a mismatch the job was ran a third time to establish a match").
+ * pairings_vote_rows compares n_words words (HOST): returns 0 if a == b, or if c (the third run, may be NULL) equals
+ * a; 1 if c equals b (b stands); 3 if a != b and c is NULL (a third run is needed); PAIRINGS_ECHECK if no two of the
+ * three agree.  pairings_duplicate_vote drives it: eval(ctx, attempt, rows) must fill n_words words for attempt 0 and
+ * 1, and 2 only after a mismatch (attempts should differ in how they compute: other GPU, other launch geometry,
+ * other kernel); rows_out receives the rows two runs agreed on, *mismatch_out (may be NULL) 1 if the first two
+ * differed.  A non-zero return of eval is passed through.  Host only; pairings_run_ex uses it. */
+typedef int (*pairings_eval_fn)(void* ctx, int attempt, uint32_t* rows_out);
+int pairings_vote_rows(const uint32_t* a, const uint32_t* b, const uint32_t* c, uint64_t n_words);
+int pairings_duplicate_vote(pairings_eval_fn eval, void* ctx, uint64_t n_words, uint32_t* rows_out, int* mismatch_out);
 
 /* Whole-job host driver: partition -> count_pairings_host per range -> sum rows -> journal.
  * Skips ranges already in the journal (journal_path may be NULL = no journal).  Stops after
@@ -207,14 +232,35 @@ int pairings_lemma24(int kind, int n);
  * time with another launch geometry (another Gray-bit count: another thread <-> term mapping and summation
  * order) — and the rows are compared word by word; on a mismatch a third run decides, and if no two runs
  * agree the call fails with PAIRINGS_ECHECK.  *duplicate_mismatches_out (may be NULL) counts the ranges
- * whose first two runs disagreed.  Costs twice the time. */
-enum { PAIRINGS_RUN_LEMMA24 = 1, PAIRINGS_RUN_DUPLICATE = 2 };
+ * whose first two runs disagreed.  Costs twice the time.
+ *
+ * PAIRINGS_RUN_AUDIT: a cheap second opinion from an independent implementation — of every chunk range, the first
+ * chunk and one seeded chunk are evaluated again by PAIRINGS_VARIANT_GENERIC (other kernel, other arithmetic: per-term
+ * Montgomery residues instead of exact multi-word sums) and compared word by word; on a mismatch a third run of that
+ * chunk (the fast kernel at another Gray-bit count) votes: if it sides with the fast kernel the range stands (the
+ * mismatch is counted), otherwise the call fails with PAIRINGS_ECHECK.  Costs a few per cent. */
+enum { PAIRINGS_RUN_LEMMA24 = 1, PAIRINGS_RUN_DUPLICATE = 2, PAIRINGS_RUN_AUDIT = 4 };
 int pairings_run_ex(int kind, int n, int chunk_bits,
                     const uint32_t* moduli, int n_moduli,
                     uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
                     void* stream, const pairings_launch_opts* opts, unsigned flags,
                     uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
                     uint64_t* duplicate_mismatches_out);
+
+/* One job of a chunk farm ("split ... into several independent sets and simply put the result together
+ * at the end"; S(25) as 4 GPU jobs, L(27) 64, n = 28 256, S(29) 1024): pairings_run_ex restricted to the
+ * chunks of [slice_begin, slice_end) (within [0, 2^chunk_bits); with PAIRINGS_RUN_LEMMA24 only the part below
+ * 2^{chunk_bits-1} is evaluated).  total_out = the summed rows of the slice (never doubled: the symmetry factor belongs
+ * to the whole job and is applied by whoever adds the slices up), *chunks_needed_out = chunks of the slice this mode
+ * evaluates.  A journal holding ranges outside the slice is refused (PAIRINGS_EJOURNAL).  The slices of the ranks come
+ * from pairings_rank_range, their journals are put together by pairings_journal_merge. */
+int pairings_run_slice(int kind, int n, int chunk_bits,
+                       const uint32_t* moduli, int n_moduli,
+                       uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                       void* stream, const pairings_launch_opts* opts, unsigned flags,
+                       uint64_t slice_begin, uint64_t slice_end,
+                       uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                       uint64_t* duplicate_mismatches_out);
 
 /* §8(a) row a7 — CRT reconstruction ("the actual value is obtained using the chinese
  * remainder theorem") and the exact division of Lemma 2.1.
@@ -255,7 +301,8 @@ int pairings_crt_signed(const uint32_t* moduli, int n_moduli, const uint32_t* re
  * Random numbers: draw(seed, ctr) = splitmix64_mix(seed + 0x9E3779B97F4A7C15 (ctr + 1)), counter layout and
  * the integer decision rule "u < floor(p 2^32)" as in DESIGN.md (readings C2, C3): the counters depend only on
  * (kind, n, betas, replica range, iterations, seed) — not on the launch — and add up over disjoint replica
- * ranges, which is how the work is sharded over calls or GPUs.  iterations <= 2^25, replica_end <= 2^30.
+ * ranges, which is how the work is sharded over calls or GPUs.  iterations <= 2^25, replica_end <= 2^30, and
+ * replica_end * (iterations + 1) * n_levels * max(n, 3) < 2^64 (the draw counter must not wrap: PAIRINGS_EINVAL_OPTS).
  * Invalid arguments are reported before anything is enqueued; the call synchronises the stream once (the
  * threshold table is staged from host memory) and then returns with the kernel enqueued. */
 #define PAIRINGS_PT_MAX_LEVELS 32
@@ -280,13 +327,6 @@ int pairings_pt_ladder(int kind, int n, double target_exchange, uint64_t pilot_r
  * PAIRINGS_ERANGE if a level has no samples or a ratio is estimated as zero. */
 int pairings_pt_estimate(int kind, int n, const double* betas, int n_levels, const uint64_t* hist_host,
                          double* ratios_out, double* log_distinct_out);
-
-/* Measurement helper (not on the path): enqueues an integer-issue calibration kernel — independent
- * chains (ILP 8) of mode 0: IADD3, 1: LOP3, 2: IMAD, 3: IADD3:IMAD 1:1 — and reports how many
- * thread-instructions of that class it executes, for the roofline denominator.
- * out_dev: DEVICE, at least one uint32 (scratch). */
-int pairings_issue_probe(int mode, int blocks, int threads, int iters, uint32_t* out_dev, void* stream,
-                         uint64_t* thread_instructions);
 
 const char* pairings_strerror(int code);
 

@@ -9,9 +9,10 @@ from .api import (  # noqa: F401
     count_pairings, count_pairings_ex, count_pairings_host, pairings_has_swar, pairings_query_geometry,
     pairings_default_moduli, pairings_min_moduli, pairings_bound_moduli,
     pairings_partition, pairings_rank_range, pairings_sum_rows,
-    pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_lemma24, RUN_LEMMA24, RUN_DUPLICATE,
+    pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_run_slice, pairings_lemma24,
+    RUN_LEMMA24, RUN_DUPLICATE, RUN_AUDIT, pairings_journal_merge, pairings_vote_rows, pairings_duplicate_vote,
     default_chunk_bits, default_chunks_per_call,
     pairings_reconstruct, pairings_crt_signed, pairings_strerror, pairings_build_info,
-    pairings_issue_probe, pairings_pt_run, pairings_pt_estimate, pairings_pt_ladder,
+    pairings_pt_run, pairings_pt_estimate, pairings_pt_ladder,
     count, approx_count,
 )

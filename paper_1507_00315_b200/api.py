@@ -22,6 +22,10 @@ class LaunchOpts(ctypes.Structure):
                 ("blocks_per_chunk", ctypes.c_int), ("nonzero_terms", ctypes.c_void_p)]
 
 
+# int (*pairings_eval_fn)(void* ctx, int attempt, uint32_t* rows_out)
+EVAL_FN = ctypes.CFUNCTYPE(ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.POINTER(ctypes.c_uint32))
+
+
 class PairingsError(RuntimeError):
     def __init__(self, code: int, where: str):
         self.code = code
@@ -63,6 +67,11 @@ def lib():
         "pairings_journal_load": (ctypes.c_int64, [cp, i, i, i, u32p, i, u64p, ctypes.c_int64, u32p]),
         "pairings_run": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, u32p, u64p]),
         "pairings_run_ex": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, ctypes.c_uint, u32p, u64p, u64p, u64p]),
+        "pairings_run_slice": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, ctypes.c_uint, u64, u64, u32p, u64p, u64p,
+                                   u64p]),
+        "pairings_journal_merge": (ctypes.c_int64, [ctypes.POINTER(cp), i, cp, i, i, i, u32p, i, u32p, u64p]),
+        "pairings_vote_rows": (i, [u32p, u32p, u32p, u64]),
+        "pairings_duplicate_vote": (i, [EVAL_FN, vp, u64, u32p, ctypes.POINTER(i)]),
         "pairings_lemma24": (i, [i, i]),
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
@@ -70,7 +79,6 @@ def lib():
         "pairings_pt_ladder": (i, [i, i, ctypes.c_double, u64, u64, u64, ctypes.POINTER(ctypes.c_double), i, vp]),
         "pairings_pt_estimate": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64p, ctypes.POINTER(ctypes.c_double),
                                      ctypes.POINTER(ctypes.c_double)]),
-        "pairings_issue_probe": (i, [i, i, i, i, vp, vp, u64p]),
         "pairings_strerror": (cp, [i]),
         "pairings_build_info": (cp, []),
     }
@@ -216,7 +224,7 @@ def pairings_run(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=None
     return [int(t[j]) for j in range(k)], int(done.value)
 
 
-RUN_LEMMA24, RUN_DUPLICATE = 1, 2
+RUN_LEMMA24, RUN_DUPLICATE, RUN_AUDIT = 1, 2, 4
 
 
 def pairings_lemma24(kind: int, n: int) -> int:
@@ -239,6 +247,55 @@ def pairings_run_ex(kind, n, chunk_bits, moduli, chunks_per_call, journal_path=N
     return [int(t[j]) for j in range(k)], int(done.value), int(needed.value)
 
 
+def pairings_run_slice(kind, n, chunk_bits, moduli, chunks_per_call, slice_begin, slice_end, journal_path=None, max_calls=0,
+                       stream: int = 0, opts: Optional[LaunchOpts] = None, flags: int = 0):
+    """One job of a chunk farm: pairings_run_ex over the chunks of [slice_begin, slice_end) only.  Returns (summed
+    rows of the slice, chunks done, chunks this slice needs); mismatches in pairings_run_slice.last_mismatches."""
+    k = len(moduli)
+    t = _u32([0] * k)
+    done, needed, mism = ctypes.c_uint64(0), ctypes.c_uint64(0), ctypes.c_uint64(0)
+    jp = os.fsencode(journal_path) if journal_path is not None else None
+    _check(lib().pairings_run_slice(kind, n, chunk_bits, _u32(moduli), k, chunks_per_call, jp, max_calls,
+                                    ctypes.c_void_p(stream), _opts(opts), flags, slice_begin, slice_end, t,
+                                    ctypes.byref(done), ctypes.byref(needed), ctypes.byref(mism)), "pairings_run_slice")
+    pairings_run_slice.last_mismatches = int(mism.value)
+    return [int(t[j]) for j in range(k)], int(done.value), int(needed.value)
+
+
+def pairings_journal_merge(paths, kind, n, chunk_bits, moduli, out_path=None):
+    """Adds up the journals of several jobs.  Returns (ranges, total residues, chunks covered)."""
+    k = len(moduli)
+    arr = (ctypes.c_char_p * len(paths))(*[os.fsencode(p) for p in paths])
+    t = _u32([0] * k)
+    cov = ctypes.c_uint64(0)
+    nr = _check(lib().pairings_journal_merge(arr, len(paths), os.fsencode(out_path) if out_path is not None else None,
+                                             kind, n, chunk_bits, _u32(moduli), k, t, ctypes.byref(cov)),
+                "pairings_journal_merge")
+    return int(nr), [int(t[j]) for j in range(k)], int(cov.value)
+
+
+def pairings_vote_rows(a, b, c=None) -> int:
+    """0: a stands, 1: b stands, 3: a != b and no third run given; raises PairingsError(ECHECK) if no two agree."""
+    return _check(lib().pairings_vote_rows(_u32(a), _u32(b), _u32(c) if c is not None else None, len(a)),
+                  "pairings_vote_rows")
+
+
+def pairings_duplicate_vote(evaluate, n_words: int):
+    """evaluate(attempt) -> list of n_words ints (or a negative error code).  Returns (rows, mismatch)."""
+    def thunk(_ctx, attempt, out):
+        r = evaluate(int(attempt))
+        if isinstance(r, int):
+            return r
+        for j, v in enumerate(r):
+            out[j] = v
+        return 0
+    cb = EVAL_FN(thunk)
+    rows = (ctypes.c_uint32 * max(n_words, 1))()
+    mm = ctypes.c_int(0)
+    _check(lib().pairings_duplicate_vote(cb, None, n_words, rows, ctypes.byref(mm)), "pairings_duplicate_vote")
+    return [int(rows[j]) for j in range(n_words)], int(mm.value)
+
+
 def pairings_reconstruct(kind, n, moduli, total_residues):
     """Returns (D, S) = (reflections distinct, reflections identified) as Python ints."""
     a, b = ctypes.create_string_buffer(_CAP), ctypes.create_string_buffer(_CAP)
@@ -251,14 +308,6 @@ def pairings_crt_signed(moduli, residues) -> int:
     a = ctypes.create_string_buffer(_CAP)
     _check(lib().pairings_crt_signed(_u32(moduli), len(moduli), _u32(residues), a, _CAP), "pairings_crt_signed")
     return int(a.value)
-
-
-def pairings_issue_probe(mode: int, blocks: int, threads: int, iters: int, out_dev_ptr: int, stream: int = 0) -> int:
-    """Enqueues the calibration kernel; returns the number of thread-instructions it executes."""
-    cnt = ctypes.c_uint64(0)
-    _check(lib().pairings_issue_probe(mode, blocks, threads, iters, ctypes.c_void_p(out_dev_ptr),
-                                      ctypes.c_void_p(stream), ctypes.byref(cnt)), "pairings_issue_probe")
-    return int(cnt.value)
 
 
 def pairings_pt_run(kind, n, betas, replica_begin, replica_end, iterations, burn_in, seed, hist_dev_ptr: int,

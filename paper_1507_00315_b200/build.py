@@ -17,6 +17,8 @@ CSRC = os.path.join(HERE, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 OBJ = os.path.join(HERE, "build")
 SO = os.path.join(HERE, "libpairings_b200.so")
+PROBE_SRC = os.path.join(HERE, "probe", "issue_probe.cu")
+PROBE_SO = os.path.join(HERE, "libpairings_probe.so")     # bench.py's calibration kernels, not part of the product
 
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
@@ -85,5 +87,18 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return SO
 
 
+def build_probe(force: bool = False) -> str:
+    """bench.py's integer-issue calibration kernels (probe/issue_probe.cu) as their own small library."""
+    if force or not os.path.exists(PROBE_SO) or os.path.getmtime(PROBE_SO) < os.path.getmtime(PROBE_SRC):
+        tmp = PROBE_SO + ".tmp.%d" % os.getpid()
+        cmd = [NVCC] + ARCH + ["-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC", "-shared", "-o", tmp, PROBE_SRC, "-lcudart"]
+        r = subprocess.run(cmd, capture_output=True, text=True)
+        if r.returncode != 0:
+            raise RuntimeError("nvcc failed for %s:\n%s\n%s" % (PROBE_SRC, r.stdout, r.stderr))
+        os.replace(tmp, PROBE_SO)
+    return PROBE_SO
+
+
 if __name__ == "__main__":
     print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build_probe(force="--force" in sys.argv))

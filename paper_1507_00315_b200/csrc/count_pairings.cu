@@ -199,7 +199,7 @@ static int choose_geometry(int kind, int n, int chunk_bits, uint64_t n_chunks,
     if (variant == PAIRINGS_VARIANT_SWAR) return PAIRINGS_EINVAL_OPTS;
 
     // ---- generic
-    const int gmax = std::min(tb, 40);
+    const int gmax = std::min(tb, 32);                    // 2^g residues below 2^31 plus the 2^62 carried between prefixes stay below 2^64
     if (g != 0) { if (g > gmax) return PAIRINGS_EINVAL_OPTS; }
     else g = std::max(0, std::min(total_bits - 20, std::min(gmax, 12)));
     if (threads == 0) {
@@ -352,15 +352,16 @@ int count_pairings_host(int kind, int n, int chunk_bits, uint64_t chunk_begin, u
     return PAIRINGS_OK;
 }
 
-int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
-                    uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
-                    void* stream, const pairings_launch_opts* opts, unsigned flags,
-                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
-                    uint64_t* duplicate_mismatches_out) {
-    int rc = validate(kind, n, chunk_bits, 0, 0, moduli, n_moduli, total_out); if (rc) return rc;
+int pairings_run_slice(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                       uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                       void* stream, const pairings_launch_opts* opts, unsigned flags,
+                       uint64_t slice_begin, uint64_t slice_end,
+                       uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                       uint64_t* duplicate_mismatches_out) {
+    int rc = validate(kind, n, chunk_bits, slice_begin, slice_end, moduli, n_moduli, total_out); if (rc) return rc;
     if (!total_out || !chunks_done_out) return PAIRINGS_ENULL;
     if (chunks_per_call == 0) return PAIRINGS_EINVAL_CHUNK;
-    if (flags & ~(unsigned)(PAIRINGS_RUN_LEMMA24 | PAIRINGS_RUN_DUPLICATE)) return PAIRINGS_EINVAL_OPTS;
+    if (flags & ~(unsigned)(PAIRINGS_RUN_LEMMA24 | PAIRINGS_RUN_DUPLICATE | PAIRINGS_RUN_AUDIT)) return PAIRINGS_EINVAL_OPTS;
     for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
     *chunks_done_out = 0;
     if (duplicate_mismatches_out) *duplicate_mismatches_out = 0;
@@ -376,8 +377,11 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
         if (sym == 1) { needed >>= 1; multiplier = 2; }
         else { needed = 0; multiplier = 0; }           // the two halves cancel: H = 0, nothing to evaluate
     }
-    if (chunks_needed_out) *chunks_needed_out = needed;
-    if (needed == 0) return PAIRINGS_OK;
+    // a slice (one job of a chunk farm): only chunks of [slice_begin, slice_end) that this mode evaluates
+    const uint64_t sb = std::min(slice_begin, needed), se = std::min(slice_end, needed);
+    const bool whole = (sb == 0 && se == needed);
+    if (chunks_needed_out) *chunks_needed_out = se - sb;
+    if (se == sb) return PAIRINGS_OK;
 
     // a1: what is already journalled
     std::vector<uint64_t> done;
@@ -391,10 +395,12 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
         done.resize((size_t)(2 * nd));
         for (int64_t j = 0; j < nd; j++) {
             if (done[(size_t)(2 * j + 1)] > needed) return PAIRINGS_EJOURNAL;   // journal of a run without the symmetry
+            if (done[(size_t)(2 * j)] < sb || done[(size_t)(2 * j + 1)] > se) return PAIRINGS_EJOURNAL;   // journal of another slice
             *chunks_done_out += done[(size_t)(2 * j + 1)] - done[(size_t)(2 * j)];
         }
     }
-    if (needed < (1ULL << chunk_bits)) { done.push_back(needed); done.push_back(1ULL << chunk_bits); }   // not to be evaluated
+    if (se < (1ULL << chunk_bits)) { done.push_back(se); done.push_back(1ULL << chunk_bits); }   // not to be evaluated
+    if (sb > 0) { done.push_back(0); done.push_back(sb); }
     // a1: the remaining ranges
     int64_t need = pairings_partition(chunk_bits, chunks_per_call, done.data(), (int)(done.size() / 2), nullptr, 0);
     if (need < 0) return (int)need;
@@ -402,40 +408,58 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
     need = pairings_partition(chunk_bits, chunks_per_call, done.data(), (int)(done.size() / 2), ranges.data(), need);
     if (need < 0) return (int)need;
 
-    std::vector<uint32_t> rows, rows_dup;
+    std::vector<uint32_t> rows;
     int64_t calls = 0;
     for (int64_t r = 0; r < need; r++) {
         if (max_calls > 0 && calls >= max_calls) break;
         const uint64_t b = ranges[(size_t)(2 * r)], e = ranges[(size_t)(2 * r + 1)];
         rows.resize((size_t)(e - b) * (size_t)n_moduli);
-        rc = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, rows.data(), stream, opts);
-        if (rc) return rc;
-        if (flags & PAIRINGS_RUN_DUPLICATE) {
-            // "every GPU job run twice ... a third run on mismatch" (silent GPU errors).  With one
-            // GPU the second run uses another launch geometry (other Gray-bit count: other thread <-> term
-            // mapping, other summation order), so a repeatable fault of one mapping does not hide itself.
-            Geometry geo; rc = choose_geometry(kind, n, chunk_bits, e - b, opts, &geo); if (rc) return rc;
+        // another launch geometry of the same kernel variant: the nearest admissible Gray-bit count (other thread <->
+        // term mapping, other summation order); if none exists (tiny jobs) the same geometry again
+        auto rerun_other_geometry = [&](int first_dg, uint64_t rb, uint64_t re, uint32_t* dst) -> int {
+            Geometry geo; int rc2 = choose_geometry(kind, n, chunk_bits, re - rb, opts, &geo); if (rc2) return rc2;
             pairings_launch_opts alt; std::memset(&alt, 0, sizeof alt);
             alt.variant = geo.variant;
-            auto rerun = [&](int first_dg, std::vector<uint32_t>& dst) -> int {
-                dst.resize(rows.size());
-                int rc2 = PAIRINGS_EINVAL_OPTS;
-                for (int dg = first_dg; dg <= first_dg + 4 && rc2 == PAIRINGS_EINVAL_OPTS; dg += 2) {   // nearest admissible g
-                    alt.gray_bits = geo.g - dg > 0 ? geo.g - dg : geo.g + dg;
-                    rc2 = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, dst.data(), stream, &alt);
-                }
-                if (rc2 == PAIRINGS_EINVAL_OPTS)                      // no other geometry exists (tiny jobs): the same one again
-                    rc2 = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, dst.data(), stream, opts);
-                return rc2;
+            rc2 = PAIRINGS_EINVAL_OPTS;
+            for (int dg = first_dg; dg <= first_dg + 4 && rc2 == PAIRINGS_EINVAL_OPTS; dg += 2) {
+                alt.gray_bits = geo.g - dg > 0 ? geo.g - dg : geo.g + dg;
+                rc2 = count_pairings_host(kind, n, chunk_bits, rb, re, moduli, n_moduli, dst, stream, &alt);
+            }
+            if (rc2 == PAIRINGS_EINVAL_OPTS) rc2 = count_pairings_host(kind, n, chunk_bits, rb, re, moduli, n_moduli, dst, stream, opts);
+            return rc2;
+        };
+        if (flags & PAIRINGS_RUN_DUPLICATE) {
+            // "every GPU job was ran twice ... a third time to establish a match" (silent GPU errors).  With
+            // one GPU the second and third runs use other launch geometries, so a repeatable fault of one mapping does
+            // not hide itself.  The vote itself is pairings_duplicate_vote (host_math.cpp).
+            struct Ctx { decltype(rerun_other_geometry)* rerun; uint64_t b, e; int kind, n, C; const uint32_t* moduli; int m;
+                         void* stream; const pairings_launch_opts* opts; } ctx{&rerun_other_geometry, b, e, kind, n, chunk_bits, moduli, n_moduli, stream, opts};
+            auto eval = [](void* c, int attempt, uint32_t* out) -> int {
+                Ctx* x = static_cast<Ctx*>(c);
+                if (attempt == 0) return count_pairings_host(x->kind, x->n, x->C, x->b, x->e, x->moduli, x->m, out, x->stream, x->opts);
+                return (*x->rerun)(attempt, x->b, x->e, out);
             };
-            rc = rerun(1, rows_dup); if (rc) return rc;
-            if (std::memcmp(rows.data(), rows_dup.data(), rows.size() * sizeof(uint32_t)) != 0) {
+            int mismatch = 0;
+            rc = pairings_duplicate_vote(eval, &ctx, (uint64_t)rows.size(), rows.data(), &mismatch); if (rc) return rc;
+            if (mismatch && duplicate_mismatches_out) ++*duplicate_mismatches_out;
+        } else {
+            rc = count_pairings_host(kind, n, chunk_bits, b, e, moduli, n_moduli, rows.data(), stream, opts);
+            if (rc) return rc;
+        }
+        if (flags & PAIRINGS_RUN_AUDIT) {
+            // the generic kernel as auditor of the first and of one seeded chunk of the range
+            uint64_t z = b * 0x9E3779B97F4A7C15ULL + 0xD1B54A32D192ED03ULL; z ^= z >> 29; z *= 0xBF58476D1CE4E5B9ULL; z ^= z >> 32;
+            const uint64_t picks[2] = {b, b + z % (e - b)};
+            pairings_launch_opts gen; std::memset(&gen, 0, sizeof gen); gen.variant = PAIRINGS_VARIANT_GENERIC;
+            for (int a = 0; a < (picks[1] == picks[0] ? 1 : 2); a++) {
+                const uint64_t c = picks[a];
+                uint32_t second[PAIRINGS_MAX_MODULI], third[PAIRINGS_MAX_MODULI];
+                rc = count_pairings_host(kind, n, chunk_bits, c, c + 1, moduli, n_moduli, second, stream, &gen); if (rc) return rc;
+                const uint32_t* first = rows.data() + (size_t)(c - b) * (size_t)n_moduli;
+                if (pairings_vote_rows(first, second, nullptr, (uint64_t)n_moduli) == 0) continue;
                 if (duplicate_mismatches_out) ++*duplicate_mismatches_out;
-                std::vector<uint32_t> third;
-                rc = rerun(2, third); if (rc) return rc;
-                if (std::memcmp(third.data(), rows.data(), rows.size() * sizeof(uint32_t)) == 0) { /* first run stands */ }
-                else if (std::memcmp(third.data(), rows_dup.data(), rows.size() * sizeof(uint32_t)) == 0) rows.swap(rows_dup);
-                else return PAIRINGS_ECHECK;                          // three runs, no two agree
+                rc = rerun_other_geometry(1, c, c + 1, third); if (rc) return rc;
+                if (pairings_vote_rows(first, second, third, (uint64_t)n_moduli) != 0) return PAIRINGS_ECHECK;
             }
         }
         uint32_t row_sum[PAIRINGS_MAX_MODULI] = {0};
@@ -448,10 +472,21 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
         *chunks_done_out += e - b;
         calls++;
     }
-    if (*chunks_done_out == needed && multiplier == 2) {       // complete: H = 2 * (x_2 = +1 half)
+    if (whole && *chunks_done_out == needed && multiplier == 2) {       // complete: H = 2 * (x_2 = +1 half)
         rc = pairings_sum_rows(total_out, 1, moduli, n_moduli, total_out); if (rc) return rc;
     }
     return PAIRINGS_OK;
+}
+
+int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                    uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                    void* stream, const pairings_launch_opts* opts, unsigned flags,
+                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                    uint64_t* duplicate_mismatches_out) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
+    return pairings_run_slice(kind, n, chunk_bits, moduli, n_moduli, chunks_per_call, journal_path, max_calls, stream, opts,
+                              flags, 0, 1ULL << chunk_bits, total_out, chunks_done_out, chunks_needed_out, duplicate_mismatches_out);
 }
 
 int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,

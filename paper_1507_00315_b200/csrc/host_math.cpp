@@ -12,6 +12,9 @@
 #include <string>
 #include <vector>
 
+#include <fcntl.h>
+#include <unistd.h>
+
 namespace pairings {
 
 // ------------------------------------------------------------------------------------------------
@@ -320,14 +323,20 @@ static std::string journal_header(int kind, int n, int chunk_bits, const uint32_
     return h;
 }
 
-// reads complete lines (a trailing line without '\n' is a torn write and is dropped)
-static int read_lines(const char* path, std::vector<std::string>& lines, bool* exists) {
+// reads complete lines (a trailing line without '\n' is a torn write and is dropped); *complete_bytes = length of
+// the file up to and including its last '\n'
+static int read_lines(const char* path, std::vector<std::string>& lines, bool* exists, size_t* complete_bytes = nullptr,
+                      size_t* file_bytes = nullptr) {
     FILE* f = std::fopen(path, "rb");
+    if (complete_bytes) *complete_bytes = 0;
+    if (file_bytes) *file_bytes = 0;
     if (!f) { *exists = false; return errno == ENOENT ? PAIRINGS_OK : PAIRINGS_EJOURNAL; }
     *exists = true;
     std::string data; char buf[65536]; size_t got;
     while ((got = std::fread(buf, 1, sizeof buf, f)) > 0) data.append(buf, got);
+    const bool bad = std::ferror(f) != 0;
     std::fclose(f);
+    if (bad) return PAIRINGS_EJOURNAL;
     size_t pos = 0;
     while (true) {
         size_t nl = data.find('\n', pos);
@@ -335,6 +344,64 @@ static int read_lines(const char* path, std::vector<std::string>& lines, bool* e
         lines.emplace_back(data.substr(pos, nl - pos));
         pos = nl + 1;
     }
+    if (complete_bytes) *complete_bytes = pos;
+    if (file_bytes) *file_bytes = data.size();
+    return PAIRINGS_OK;
+}
+
+// one unsigned decimal token (digits only: no sign, no 0x) followed by a blank or the end of the line
+static bool next_u64(const char*& s, unsigned long long* out) {
+    while (*s == ' ') s++;
+    if (*s < '0' || *s > '9') return false;
+    unsigned long long v = 0;
+    int digits = 0;
+    while (*s >= '0' && *s <= '9') {
+        if (++digits > 20 || v > (~0ULL - (unsigned)(*s - '0')) / 10ULL) return false;   // would not fit 64 bits
+        v = v * 10ULL + (unsigned)(*s - '0');
+        s++;
+    }
+    if (*s != ' ' && *s != '\0') return false;
+    *out = v;
+    return true;
+}
+
+struct JournalLine { uint64_t b, e; uint32_t row[PAIRINGS_MAX_MODULI]; };
+
+// "begin end r_0 .. r_{m-1}", nothing else on the line
+static bool parse_journal_line(const std::string& line, int n_moduli, const uint32_t* moduli, uint64_t total, JournalLine* out) {
+    const char* s = line.c_str();
+    unsigned long long b, e, v;
+    if (!next_u64(s, &b) || !next_u64(s, &e)) return false;
+    if (b >= e || e > total) return false;
+    out->b = b; out->e = e;
+    for (int i = 0; i < n_moduli; i++) {
+        if (!next_u64(s, &v) || v >= moduli[i]) return false;
+        out->row[i] = (uint32_t)v;
+    }
+    while (*s == ' ') s++;
+    return *s == '\0';                     // trailing tokens: two lines glued together, or another file format
+}
+
+// all data lines of a journal, checked: header, syntax, ranges inside [0, 2^C), no two ranges overlap
+static int load_journal(const char* path, int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                        std::vector<JournalLine>& out, bool* exists_out = nullptr) {
+    std::vector<std::string> lines; bool exists = false;
+    int rc = read_lines(path, lines, &exists); if (rc) return rc;
+    if (exists_out) *exists_out = exists;
+    if (!exists || lines.empty()) return PAIRINGS_OK;
+    if (lines[0] != journal_header(kind, n, chunk_bits, moduli, n_moduli)) return PAIRINGS_EJOURNAL;
+    const uint64_t total = 1ULL << chunk_bits;
+    out.reserve(lines.size());
+    for (size_t li = 1; li < lines.size(); li++) {
+        JournalLine jl;
+        if (!parse_journal_line(lines[li], n_moduli, moduli, total, &jl)) return PAIRINGS_EJOURNAL;
+        out.push_back(jl);
+    }
+    // overlap = double count: sort a copy of the ranges by begin, neighbours must not intersect
+    std::vector<std::pair<uint64_t, uint64_t>> r; r.reserve(out.size());
+    for (auto& jl : out) r.emplace_back(jl.b, jl.e);
+    std::sort(r.begin(), r.end());
+    for (size_t i = 1; i < r.size(); i++) if (r[i].first < r[i - 1].second) return PAIRINGS_EJOURNAL;
     return PAIRINGS_OK;
 }
 
@@ -346,31 +413,33 @@ int64_t pairings_journal_load(const char* path, int kind, int n, int chunk_bits,
     rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
     if (!path || !total_out || (cap_ranges > 0 && !out_ranges)) return PAIRINGS_ENULL;
     for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
-    std::vector<std::string> lines; bool exists = false;
-    rc = read_lines(path, lines, &exists); if (rc) return rc;
-    if (!exists || lines.empty()) return 0;
-    if (lines[0] != journal_header(kind, n, chunk_bits, moduli, n_moduli)) return PAIRINGS_EJOURNAL;
-    const uint64_t total = 1ULL << chunk_bits;
+    std::vector<JournalLine> lines;
+    rc = load_journal(path, kind, n, chunk_bits, moduli, n_moduli, lines); if (rc) return rc;
     int64_t count = 0;
-    std::vector<std::pair<uint64_t, uint64_t>> seen;
-    for (size_t li = 1; li < lines.size(); li++) {
-        const char* s = lines[li].c_str(); char* endp = nullptr;
-        unsigned long long b = std::strtoull(s, &endp, 10); if (endp == s) return PAIRINGS_EJOURNAL; s = endp;
-        unsigned long long e = std::strtoull(s, &endp, 10); if (endp == s) return PAIRINGS_EJOURNAL; s = endp;
-        if (b >= e || e > total) return PAIRINGS_EJOURNAL;
-        for (auto& r : seen) if (b < r.second && r.first < e) return PAIRINGS_EJOURNAL;  // overlap = double count
-        uint32_t row[PAIRINGS_MAX_MODULI];
-        for (int i = 0; i < n_moduli; i++) {
-            unsigned long long v = std::strtoull(s, &endp, 10); if (endp == s) return PAIRINGS_EJOURNAL; s = endp;
-            if (v >= moduli[i]) return PAIRINGS_EJOURNAL;
-            row[i] = (uint32_t)v;
-        }
-        seen.emplace_back(b, e);
-        pairings_sum_rows(row, 1, moduli, n_moduli, total_out);
-        if (count < cap_ranges) { out_ranges[2 * count] = b; out_ranges[2 * count + 1] = e; }
+    for (auto& jl : lines) {
+        pairings_sum_rows(jl.row, 1, moduli, n_moduli, total_out);
+        if (count < cap_ranges) { out_ranges[2 * count] = jl.b; out_ranges[2 * count + 1] = jl.e; }
         count++;
     }
     return count;
+}
+
+static std::string format_journal_line(uint64_t b, uint64_t e, const uint32_t* row, int n_moduli) {
+    std::string line = std::to_string(b) + " " + std::to_string(e);
+    for (int i = 0; i < n_moduli; i++) line += " " + std::to_string(row[i]);
+    line += "\n";
+    return line;
+}
+
+// write + flush + fsync; the data must be on disk before the caller counts the range as done
+static int write_all_sync(int fd, const std::string& data) {
+    size_t off = 0;
+    while (off < data.size()) {
+        ssize_t w = ::write(fd, data.data() + off, data.size() - off);
+        if (w < 0) { if (errno == EINTR) continue; return PAIRINGS_EJOURNAL; }
+        off += (size_t)w;
+    }
+    return ::fsync(fd) == 0 ? PAIRINGS_OK : PAIRINGS_EJOURNAL;
 }
 
 int pairings_journal_append(const char* path, int kind, int n, int chunk_bits,
@@ -382,22 +451,86 @@ int pairings_journal_append(const char* path, int kind, int n, int chunk_bits,
     if (!path || !row_sum) return PAIRINGS_ENULL;
     if (chunk_begin == chunk_end) return PAIRINGS_EINVAL_CHUNK;
     for (int i = 0; i < n_moduli; i++) if (row_sum[i] >= moduli[i]) return PAIRINGS_EINVAL_MODULUS;
-    std::vector<std::string> lines; bool exists = false;
-    rc = read_lines(path, lines, &exists); if (rc) return rc;
+    std::vector<std::string> lines; bool exists = false; size_t complete = 0, size = 0;
+    rc = read_lines(path, lines, &exists, &complete, &size); if (rc) return rc;
     const std::string header = journal_header(kind, n, chunk_bits, moduli, n_moduli);
     if (exists && !lines.empty() && lines[0] != header) return PAIRINGS_EJOURNAL;
     const bool need_header = !exists || lines.empty();
-    FILE* f = std::fopen(path, need_header ? "wb" : "ab");
-    if (!f) return PAIRINGS_EJOURNAL;
-    std::string line;
-    if (need_header) line += header + "\n";
-    line += std::to_string(chunk_begin) + " " + std::to_string(chunk_end);
-    for (int i = 0; i < n_moduli; i++) line += " " + std::to_string(row_sum[i]);
-    line += "\n";
-    size_t w = std::fwrite(line.data(), 1, line.size(), f);
-    int ok = (w == line.size()) && std::fflush(f) == 0;
-    std::fclose(f);
-    return ok ? PAIRINGS_OK : PAIRINGS_EJOURNAL;
+    // A torn last line (a crash in the middle of a write: bytes after the last '\n') is cut off first; appending
+    // behind it would glue the new line onto the fragment.  A file with no complete line at all is started afresh.
+    const int fd = ::open(path, O_WRONLY | O_CREAT, 0644);
+    if (fd < 0) return PAIRINGS_EJOURNAL;
+    const off_t keep = need_header ? 0 : (off_t)complete;
+    if ((size != (size_t)keep && ::ftruncate(fd, keep) != 0) || ::lseek(fd, keep, SEEK_SET) != keep) { ::close(fd); return PAIRINGS_EJOURNAL; }
+    std::string data;
+    if (need_header) data += header + "\n";
+    data += format_journal_line(chunk_begin, chunk_end, row_sum, n_moduli);
+    rc = write_all_sync(fd, data);
+    if (::close(fd) != 0 && rc == PAIRINGS_OK) rc = PAIRINGS_EJOURNAL;
+    return rc;
+}
+
+int64_t pairings_journal_merge(const char* const* paths, int n_paths, const char* out_path, int kind, int n, int chunk_bits,
+                               const uint32_t* moduli, int n_moduli, uint32_t* total_out, uint64_t* chunks_covered_out) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    rc = check_moduli(moduli, n_moduli); if (rc) return rc;
+    rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
+    if (!paths || n_paths < 1 || !total_out) return PAIRINGS_ENULL;
+    for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
+    std::vector<JournalLine> all;
+    for (int j = 0; j < n_paths; j++) {
+        if (!paths[j]) return PAIRINGS_ENULL;
+        std::vector<JournalLine> part; bool exists = false;
+        rc = load_journal(paths[j], kind, n, chunk_bits, moduli, n_moduli, part, &exists); if (rc) return rc;
+        if (!exists) return PAIRINGS_EJOURNAL;                      // a rank's file is missing: not "nothing done"
+        all.insert(all.end(), part.begin(), part.end());
+    }
+    std::sort(all.begin(), all.end(), [](const JournalLine& x, const JournalLine& y) { return x.b < y.b; });
+    uint64_t covered = 0;
+    for (size_t i = 0; i < all.size(); i++) {
+        if (i && all[i].b < all[i - 1].e) return PAIRINGS_EJOURNAL;   // two journals hold the same chunk: double count
+        covered += all[i].e - all[i].b;
+        pairings_sum_rows(all[i].row, 1, moduli, n_moduli, total_out);
+    }
+    if (chunks_covered_out) *chunks_covered_out = covered;
+    if (out_path) {
+        std::string data = journal_header(kind, n, chunk_bits, moduli, n_moduli) + "\n";
+        for (auto& jl : all) data += format_journal_line(jl.b, jl.e, jl.row, n_moduli);
+        const int fd = ::open(out_path, O_WRONLY | O_CREAT | O_TRUNC, 0644);
+        if (fd < 0) return PAIRINGS_EJOURNAL;
+        rc = write_all_sync(fd, data);
+        if (::close(fd) != 0 && rc == PAIRINGS_OK) rc = PAIRINGS_EJOURNAL;
+        if (rc) return rc;
+    }
+    return (int64_t)all.size();
+}
+
+int pairings_vote_rows(const uint32_t* a, const uint32_t* b, const uint32_t* c, uint64_t n_words) {
+    if (!a || !b) return PAIRINGS_ENULL;
+    const size_t bytes = (size_t)n_words * sizeof(uint32_t);
+    if (std::memcmp(a, b, bytes) == 0) return 0;                  // the two runs agree: a stands
+    if (!c) return 3;                                             // disagreement, a third run is needed
+    if (std::memcmp(c, a, bytes) == 0) return 0;                  // third run confirms the first
+    if (std::memcmp(c, b, bytes) == 0) return 1;                  // third run confirms the second
+    return PAIRINGS_ECHECK;                                       // three runs, no two agree
+}
+
+int pairings_duplicate_vote(pairings_eval_fn eval, void* ctx, uint64_t n_words, uint32_t* rows_out, int* mismatch_out) {
+    if (!eval || (n_words && !rows_out)) return PAIRINGS_ENULL;
+    if (mismatch_out) *mismatch_out = 0;
+    std::vector<uint32_t> second((size_t)n_words), third;
+    int rc = eval(ctx, 0, rows_out); if (rc) return rc;
+    rc = eval(ctx, 1, second.data()); if (rc) return rc;
+    int v = pairings_vote_rows(rows_out, second.data(), nullptr, n_words);
+    if (v == 0) return PAIRINGS_OK;
+    if (v < 0) return v;
+    if (mismatch_out) *mismatch_out = 1;                          // "ran a third time to establish a match"
+    third.resize((size_t)n_words);
+    rc = eval(ctx, 2, third.data()); if (rc) return rc;
+    v = pairings_vote_rows(rows_out, second.data(), third.data(), n_words);
+    if (v < 0) return v;
+    if (v == 1) std::memcpy(rows_out, second.data(), (size_t)n_words * sizeof(uint32_t));
+    return PAIRINGS_OK;
 }
 
 // ---- CRT -----------------------------------------------------------------------------------

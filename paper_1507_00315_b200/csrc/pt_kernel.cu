@@ -180,7 +180,12 @@ int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
                     uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream) {
     int rc = pt_check(kind, n, betas, n_levels); if (rc) return rc;
     if (replica_begin > replica_end || iterations == 0 || iterations > (1ULL << 25) || burn_in >= iterations) return PAIRINGS_EINVAL_OPTS;
-    if (replica_end > (1ULL << 30)) return PAIRINGS_EINVAL_OPTS;      // the draw counter must stay below 2^64
+    if (replica_end > (1ULL << 30)) return PAIRINGS_EINVAL_OPTS;
+    {   // the draw counter ((r (T+1) + tt) M + j) S + slot, S = max(n, 3), must stay below 2^64: otherwise it wraps and two
+        // replicas share a random stream (the oracle wraps the same way, so parity would not show it)
+        const unsigned __int128 span = (unsigned __int128)replica_end * (iterations + 1) * (unsigned)n_levels * (unsigned)(n > 3 ? n : 3);
+        if (span >> 64) return PAIRINGS_EINVAL_OPTS;
+    }
     if (!hist_dev || !moves_dev || !swaps_dev) return PAIRINGS_ENULL;
     if (replica_begin == replica_end) return PAIRINGS_OK;
     const int M = n_levels, N = 2 * n;

@@ -30,3 +30,34 @@ def test_gpu_arm_refuses_to_run_without_a_device():
     out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--steps", "1"], capture_output=True, text=True,
                          timeout=600, cwd=ROOT)
     assert out.returncode != 0 and "no CPU fallback" in (out.stderr + out.stdout)
+
+
+def test_gpus_n_starts_its_own_ranks():
+    """`bench.py --gpus 2` without torchrun spawns two ranks itself (RANK / LOCAL_RANK / WORLD_SIZE / MASTER_* set); in the
+    reference arm rank 0 alone works and prints the line, the other rank exits 0 — the launcher is what is tested here."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0"],
+                         capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+    assert out.returncode == 0, out.stderr
+    lines = [ln for ln in out.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2
+
+
+def test_world_size_must_match_gpus():
+    env = dict(os.environ, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "1", "--steps", "1"], capture_output=True, text=True,
+                         timeout=600, cwd=ROOT, env=env)
+    assert out.returncode != 0 and "WORLD_SIZE" in (out.stderr + out.stdout)
+
+
+def test_ncu_metrics_record_is_consistent():
+    """profiles/ncu_metrics.json (what bench.py's roofline.executed_instr_per_term comes from) agrees with itself."""
+    path = os.path.join(ROOT, "profiles", "ncu_metrics.json")
+    if not os.path.exists(path):
+        return
+    doc = json.load(open(path))
+    for name, m in doc["instances"].items():
+        assert abs(m["instr_per_term"] - m["inst_executed_warp"] * 32 / m["terms"]) < 1e-6, name
+        assert 0 < m["issue_active_pct"] <= 100 and m["kernel"].startswith("swar_kernel<")

@@ -327,3 +327,47 @@ def test_more_paper_totals(kind, n, paper_counts):
     full = pb.count(kind, n)
     assert full[1] == paper_counts[(kind, n)] and full[0] == 2 * full[1]
     assert pb.count(kind, n, lemma24=True, duplicate=True) == full
+
+
+# ---- the chunk farm on one GPU
+def test_slices_of_two_jobs_merge_to_the_count(tmp_path, paper_counts):
+    kind, n, C = S, 16, 10
+    moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)
+    paths = []
+    for r in range(3):                                   # three jobs over the x_2 = +1 half (symmetry 3), audited
+        b, e = pb.pairings_rank_range(C - 1, r, 3)
+        path = str(tmp_path / ("job%d.txt" % r))
+        total, done, needed = pb.pairings_run_slice(kind, n, C, moduli, 100, b, e, path, 0, 0, None, pb.RUN_LEMMA24 | pb.RUN_AUDIT)
+        assert done == needed == e - b and pb.pairings_run_slice.last_mismatches == 0
+        with pytest.raises(pb.PairingsError):            # the journal of one job is not another job's
+            pb.pairings_run_slice(kind, n, C, moduli, 100, e % (1 << (C - 1)), (e % (1 << (C - 1))) + 1, path, 0, 0, None, pb.RUN_LEMMA24)
+        paths.append(path)
+    nr, total, covered = pb.pairings_journal_merge(paths, kind, n, C, moduli)
+    assert covered == 1 << (C - 1)
+    total = pb.pairings_sum_rows([total], moduli, total)                 # H = 2 x (the x_2 = +1 half)
+    assert pb.pairings_reconstruct(kind, n, moduli, total) == (2 * paper_counts[(kind, n)], paper_counts[(kind, n)])
+    # the command line does the same: two jobs, then --merge
+    from paper_1507_00315_b200 import __main__ as cli
+    js = [str(tmp_path / ("cli%d.txt" % r)) for r in range(2)]
+    for r in range(2):
+        assert cli.main(["L", "12", "--chunk-bits", "6", "--rank", str(r), "--world", "2", "--journal", js[r], "--audit"]) == 0
+    assert cli.main(["L", "12", "--chunk-bits", "6", "--merge"] + js) == 0
+
+
+@pytest.mark.parametrize("kind,n,C", [(L, 12, 6), (S, 13, 8), (L, 16, 10)])
+def test_generic_kernel_audits_the_fast_kernel(kind, n, C, paper_counts):
+    moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)
+    total, done, needed = pb.pairings_run_ex(kind, n, C, moduli, 1 << (C - 3), None, 0, 0, None, pb.RUN_AUDIT | pb.RUN_DUPLICATE)
+    assert done == needed == 1 << C and pb.pairings_run_ex.last_mismatches == 0
+    assert pb.pairings_reconstruct(kind, n, moduli, total)[1] == paper_counts[(kind, n)]
+
+
+def test_bench_self_spawn_path_on_one_gpu():
+    import json, os, subprocess, sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--gpus", "1", "--spawn", "--steps", "1", "--no-cpu", "--no-pt",
+                          "--no-configs", "--no-n24"], capture_output=True, text=True, timeout=900, cwd=root, env=env)
+    assert out.returncode == 0, out.stderr[-2000:]
+    d = json.loads([ln for ln in out.stdout.splitlines() if ln.strip()][-1])
+    assert d["n_gpus"] == 1 and d["config"]["launcher"] == "self-spawned ranks" and d["scaling"] == "strong" and d["value"] > 1e11

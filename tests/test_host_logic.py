@@ -231,6 +231,118 @@ def test_journal_roundtrip_and_mismatch(tmp_path):
         pb.pairings_journal_load(path2, 1, 12, 6, moduli)
 
 
+def test_journal_append_after_a_torn_line_and_strict_lines(tmp_path):
+    # a crash in the middle of a write leaves bytes behind the last newline: the next append must cut them off, not
+    # glue its own line onto them (the glued line would parse as a valid range with garbage residues)
+    path = str(tmp_path / "j.txt")
+    moduli = pb.pairings_default_moduli(4)
+    pb.pairings_journal_append(path, 1, 12, 6, moduli, 0, 8, [1, 2, 3, 4])
+    with open(path, "ab") as f:
+        f.write(b"24 32 1 2")
+    pb.pairings_journal_append(path, 1, 12, 6, moduli, 32, 40, [100, 200, 300, 400])
+    ranges, total = pb.pairings_journal_load(path, 1, 12, 6, moduli)
+    assert ranges == [(0, 8), (32, 40)] and total == [101, 202, 303, 404]
+    text = open(path).read()
+    assert text.endswith("32 40 100 200 300 400\n") and "24 32" not in text
+    # a torn HEADER (no complete line at all): the file is started afresh
+    path2 = str(tmp_path / "j2.txt")
+    with open(path2, "wb") as f:
+        f.write(b"pairings-journal v1 kind=1 n=1")
+    assert pb.pairings_journal_load(path2, 1, 12, 6, moduli) == ([], [0, 0, 0, 0])
+    pb.pairings_journal_append(path2, 1, 12, 6, moduli, 8, 16, [5, 6, 7, 8])
+    assert pb.pairings_journal_load(path2, 1, 12, 6, moduli) == ([(8, 16)], [5, 6, 7, 8])
+    # lines with surplus, missing or non-numeric tokens, signs, overflowing numbers, residues >= p: refused
+    header = open(path).read().splitlines()[0]
+    for bad in ("0 8 1 2 3 4 5", "0 8 1 2 3", "0 8 1 2 x 4", "0 -8 1 2 3 4", "+0 8 1 2 3 4", "0 8 1 2 3 99999999999999999999999",
+                "0 8 1 2 3 %d" % moduli[3], "8 8 1 2 3 4", "0 65 1 2 3 4", "0x0 8 1 2 3 4", "0 8 1 2 3 4\t5", ""):
+        p3 = str(tmp_path / "bad.txt")
+        with open(p3, "w") as f:
+            f.write(header + "\n" + bad + "\n")
+        with pytest.raises(pb.PairingsError) as ei:
+            pb.pairings_journal_load(p3, 1, 12, 6, moduli)
+        assert ei.value.code == -11, bad
+    # many lines: the overlap check is sort-based (2^15 ranges load at once)
+    p4 = str(tmp_path / "big.txt")
+    with open(p4, "w") as f:
+        f.write("pairings-journal v1 kind=0 n=24 chunk_bits=20 moduli=" + ",".join(map(str, moduli)) + "\n")
+        for j in range(1 << 15):
+            f.write("%d %d 1 1 1 1\n" % (32 * j, 32 * j + 32))
+    ranges, total = pb.pairings_journal_load(p4, 0, 24, 20, moduli)
+    assert len(ranges) == 1 << 15 and total == [1 << 15] * 4
+
+
+def test_journal_merge_puts_rank_journals_together(tmp_path):
+    # PAPER.md:253 "simply put the result together at the end"; PAPER.md:257 (4 .. 1024 GPU jobs)
+    moduli = pb.pairings_default_moduli(4)
+    kind, n, C = 1, 12, 6
+    rnd = random.Random(5)
+    paths, want, rows = [], [0] * 4, {}
+    for r in range(3):
+        b, e = pb.pairings_rank_range(C, r, 3)
+        path = str(tmp_path / ("rank%d.txt" % r))
+        for lo in range(b, e, 5):
+            hi = min(lo + 5, e)
+            row = [rnd.randrange(p) for p in moduli]
+            pb.pairings_journal_append(path, kind, n, C, moduli, lo, hi, row)
+            want = [(w + v) % p for w, v, p in zip(want, row, moduli)]
+        paths.append(path)
+    out = str(tmp_path / "merged.txt")
+    nr, total, covered = pb.pairings_journal_merge(paths[::-1], kind, n, C, moduli, out)
+    assert total == want and covered == 1 << C and nr == 15
+    ranges, t2 = pb.pairings_journal_load(out, kind, n, C, moduli)
+    assert t2 == want and ranges == sorted(ranges) and ranges[0][0] == 0 and ranges[-1][1] == 1 << C
+    # partial coverage is reported, not an error
+    nr, total, covered = pb.pairings_journal_merge(paths[:2], kind, n, C, moduli)
+    assert covered == pb.pairings_rank_range(C, 1, 3)[1]
+    # the same journal twice = every chunk counted twice: refused; so are a foreign journal and a missing file
+    for bad in (paths + [paths[0]], paths + [str(tmp_path / "nothing.txt")]):
+        with pytest.raises(pb.PairingsError) as ei:
+            pb.pairings_journal_merge(bad, kind, n, C, moduli)
+        assert ei.value.code == -11
+    foreign = str(tmp_path / "foreign.txt")
+    pb.pairings_journal_append(foreign, kind, 11, C, moduli, 0, 1, [0, 0, 0, 0])
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_journal_merge([paths[0], foreign], kind, n, C, moduli)
+
+
+def test_duplicate_run_vote_all_outcomes():
+    # every job twice, "if there was a mismatch the job was ran a third time to establish a match"
+    a, b, c = [1, 2, 3, 4], [1, 2, 3, 5], [9, 9, 9, 9]
+    assert pb.pairings_vote_rows(a, list(a)) == 0
+    assert pb.pairings_vote_rows(a, b) == 3                       # third run needed
+    assert pb.pairings_vote_rows(a, b, list(a)) == 0              # third confirms the first
+    assert pb.pairings_vote_rows(a, b, list(b)) == 1              # third confirms the second
+    with pytest.raises(pb.PairingsError) as ei:
+        pb.pairings_vote_rows(a, b, c)                            # no two agree
+    assert ei.value.code == -7
+    # the driver: which attempts are evaluated, which rows win
+    for script, want_rows, want_mm, want_calls in (
+            ({0: a, 1: list(a)}, a, 0, [0, 1]),
+            ({0: a, 1: b, 2: list(a)}, a, 1, [0, 1, 2]),
+            ({0: a, 1: b, 2: list(b)}, b, 1, [0, 1, 2])):
+        calls = []
+        rows, mm = pb.pairings_duplicate_vote(lambda k: (calls.append(k), script[k])[1], 4)
+        assert (rows, mm, calls) == (want_rows, want_mm, want_calls)
+    with pytest.raises(pb.PairingsError) as ei:
+        pb.pairings_duplicate_vote(lambda k: {0: a, 1: b, 2: c}[k], 4)
+    assert ei.value.code == -7
+    with pytest.raises(pb.PairingsError) as ei:                   # an evaluation error is passed through
+        pb.pairings_duplicate_vote(lambda k: -6 if k == 1 else a, 4)
+    assert ei.value.code == -6
+
+
+def test_run_slice_argument_checks_need_no_gpu():
+    moduli = pb.pairings_default_moduli(4)
+    # a slice of a job whose halves cancel (no pairing exists): nothing to evaluate
+    assert pb.pairings_run_slice(pb.SKOLEM, 10, 8, moduli, 64, 32, 96, None, 0, 0, None, pb.RUN_LEMMA24) == ([0] * 4, 0, 0)
+    # a slice entirely in the x_2 = -1 half of a symmetric job: nothing to evaluate either
+    assert pb.pairings_run_slice(pb.SKOLEM, 12, 8, moduli, 64, 128, 256, None, 0, 0, None, pb.RUN_LEMMA24) == ([0] * 4, 0, 0)
+    for b, e in ((5, 4), (0, 257)):
+        with pytest.raises(pb.PairingsError) as ei:
+            pb.pairings_run_slice(pb.SKOLEM, 12, 8, moduli, 64, b, e)
+        assert ei.value.code == -3
+
+
 def test_compute_without_gpu_fails_loudly():
     import torch
     if torch.cuda.is_available():
@@ -260,4 +372,4 @@ def test_run_ex_without_pairings_needs_no_gpu():
     assert (total, done, needed) == ([0, 0, 0, 0], 0, 0)
     assert pb.pairings_reconstruct(pb.SKOLEM, 10, moduli, total) == (0, 0)
     with pytest.raises(pb.PairingsError):
-        pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, 4)      # unknown flag
+        pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, 8)      # unknown flag

@@ -54,3 +54,52 @@ def test_two_ranks_disjoint_ranges_then_crt(kind, n, C, want):
     assert all(p.exitcode == 0 for p in procs)
     assert (b, e) == (0, 1 << (C - 1))
     assert got == want          # L(8)=150, S(9)=1,328, S(7): no pairing
+
+
+def test_cli_merges_two_rank_journals_of_L12(tmp_path, capsys):
+    """The paper's workflow: N independent jobs, results put together afterwards.  Here the rows
+    of each rank's slice come from the CPU oracle (no GPU on this box); the journals, the merge and the CLI are the
+    product's.  L(12) = 108,144.  With symmetry 3 only the x_2 = +1 half is dealt out and doubled."""
+    import json
+    import threading
+    import oracle
+    import paper_1507_00315_b200 as pb
+    from paper_1507_00315_b200 import __main__ as cli
+    kind, n, C = pb.LANGFORD, 12, 6
+    moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)
+    rows = [None] * (1 << C)
+
+    def work(t):
+        for c in range(t, 1 << C, 8):
+            rows[c] = oracle.chunk(kind, n, C, c, moduli)[2]
+    ts = [threading.Thread(target=work, args=(t,)) for t in range(8)]
+    [t.start() for t in ts]
+    [t.join() for t in ts]
+
+    def journals(bits, tag):
+        paths = []
+        for r in range(2):
+            b, e = pb.pairings_rank_range(bits, r, 2)
+            path = str(tmp_path / ("%s_%d.txt" % (tag, r)))
+            for lo in range(b, e, 7):
+                hi = min(lo + 7, e)
+                pb.pairings_journal_append(path, kind, n, C, moduli, lo, hi, pb.pairings_sum_rows(rows[lo:hi], moduli))
+            paths.append(path)
+        return paths
+
+    full = journals(C, "full")
+    assert cli.main(["L", "12", "--chunk-bits", "6", "--json", "--merge"] + full) == 0
+    out = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert (out["identified"], out["distinct"], out["chunks_done"]) == (108144, 216288, 64)
+    half = journals(C - 1, "half")                                     # symmetry 3: chunks [0, 32) only
+    assert cli.main(["L", "12", "--chunk-bits", "6", "--lemma24", "--json", "--journal", str(tmp_path / "m.txt"), "--merge"] + half) == 0
+    out = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert (out["identified"], out["chunks_done"], out["chunks_needed"]) == (108144, 32, 32)
+    assert pb.pairings_journal_load(str(tmp_path / "m.txt"), kind, n, C, moduli)[0][-1][1] == 32
+    # one rank missing: incomplete, exit code 3, no count printed
+    assert cli.main(["L", "12", "--chunk-bits", "6", "--json", "--merge", full[0]]) == 3
+    out = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert "identified" not in out and out["chunks_done"] == 32
+    # overlapping journals (the same rank twice) and journals of the other mode are refused
+    with pytest.raises(pb.PairingsError):
+        cli.main(["L", "12", "--chunk-bits", "6", "--merge", full[0], full[0]])
