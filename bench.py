@@ -598,7 +598,7 @@ def pt_cpu_baseline():
     except Exception:                                   # no compiler on the box: report nothing rather than fail the bench
         return None
     threads = host_threads()
-    reps, its = 8, 1 << 12
+    reps, its = 256, 1 << 12                            # about 2 s of host work
     res = [None] * threads
 
     def work(t):

@@ -176,7 +176,10 @@ static int choose_geometry(int kind, int n, int chunk_bits, uint64_t n_chunks,
     if (swar_ok && g != 0 && (g < h || g > swar_gmax)) swar_ok = false;
     if (swar_ok && threads != 0 && !is_pow2((uint64_t)threads)) swar_ok = false;
     if (swar_ok) {
-        int sg = g ? g : std::max(h, std::min(total_bits - 19, std::min(swar_gmax, 14)));
+        // Gray bits per thread prefix: about 2^19 threads per launch (a few waves of blocks) with at most 2^14 steps each;
+        // small jobs take at least 2^7 steps per prefix so that the direct evaluation of the prefix (~300 instructions)
+        // and the per-thread residue reduction are amortised (measured: L(12) 28 -> 19 us, S(13) 57 -> 46 us per count)
+        int sg = g ? g : std::max(h, std::min(std::max(total_bits - 19, 7), std::min(swar_gmax, 14)));
         const int pb = tb - sg;                           // log2(prefixes per chunk) >= 5
         int st = threads ? threads : std::min(256, 1 << std::min(pb, 8));
         int sb = bpc;

@@ -782,10 +782,13 @@ template <int KIND, int NN>
 #ifndef PAIRINGS_SWAR_MINB
 #define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM (the ring limits it to 3 anyway): at most 85 registers; measured faster than 2 blocks without spills at n = 24
 #endif
+#ifndef PAIRINGS_SWAR_BIG_N
+#define PAIRINGS_SWAR_BIG_N 25   // 7-8 packed registers, 35-40 neighbour registers: 2 blocks per SM without spills (measured: S(25) +4 %, L(27) +1.5 %, S(29) +7 % over 3 blocks with spills; n = 24 is 1 % faster with 3)
+#endif
 #ifndef PAIRINGS_SWAR_MAXT
 #define PAIRINGS_SWAR_MAXT 256
 #endif
-__global__ void __launch_bounds__(PAIRINGS_SWAR_MAXT, PAIRINGS_SWAR_MINB)
+__global__ void __launch_bounds__(PAIRINGS_SWAR_MAXT, (NN >= PAIRINGS_SWAR_BIG_N ? 2 : PAIRINGS_SWAR_MINB))
 swar_kernel(const __grid_constant__ KernelParams kp) {
     using L = Lay<KIND, NN>;
     using Wk = Walker<KIND, NN>;

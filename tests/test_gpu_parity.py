@@ -307,7 +307,8 @@ def test_duplicate_run_mode_and_tight_moduli(kind, n, C, paper_counts):
 
 # ---- the remaining exact values of Tables 7/8 the SWAR kernel is compiled for
 @pytest.mark.parametrize("kind,n,C,count,pieces", [(S, 9, 4, 16, 1), (L, 15, 12, 8, 1), (S, 17, 16, 8, 1), (L, 19, 20, 8, 1),
-                                                   (L, 23, 22, 3, 16), (S, 25, 26, 3, 16), (L, 27, 30, 3, 16)])
+                                                   (L, 23, 22, 3, 16), (S, 25, 26, 3, 16), (L, 27, 30, 3, 16),
+                                                   (S, 28, 32, 3, 16), (L, 28, 32, 3, 16), (S, 29, 34, 3, 16)])
 def test_more_instances_sampled_chunks_match_oracle(kind, n, C, count, pieces):
     assert pb.pairings_has_swar(kind, n)
     moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)
