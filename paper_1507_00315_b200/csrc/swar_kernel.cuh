@@ -46,10 +46,8 @@ namespace swar {
 
 constexpr int H = PAIRINGS_SWAR_H;              // unrolled inner Gray bits
 constexpr int BLK = 1 << H;       // steps per unrolled block
-constexpr int QUAD = 4;           // steps per slot allocation and between drain checks
-constexpr int SCAP = 160;         // stack entries per warp: at most 31 left by the last drain + 32 * QUAD of one quad
-constexpr int PLANE_BYTES = SCAP * 16;   // stack = planes of 16 bytes per entry (128-bit accesses)
-static_assert(31 + 32 * QUAD < SCAP && 32 * QUAD <= 255, "stack capacity; per-quad lane prefixes are scanned in byte fields");
+constexpr int QUAD = 4;           // steps per slot allocation
+static_assert(31 * QUAD + 32 * QUAD <= 255, "per-quad lane prefixes (<= 31 * QUAD) are scanned in byte fields, and a warp total (<= 32 * QUAD) may be added to one");
 
 #define PAIRINGS_HD __host__ __device__ constexpr
 
@@ -166,6 +164,11 @@ struct Lay {
     // Plane 1 (words 4..) of a 5- or 6-word entry is COMPACT: 4 or 8 bytes per entry at that stride, so that the
     // 32-/64-bit accesses of a warp fall into distinct banks (at a 16-byte stride they are 4-/2-way conflicts —
     // measured: the shared-memory pipe, not the issue port, bounded v11).  Its address is (slot >> P1SHIFT) + k1.
+    // Drain checks: after every DQ quads.  Two quads per check (fewer checks, half the drain sites) where the stack of
+    // 31 + 256 entries still lets 3 blocks of 8 warps share an SM: one plane, or the compact plane 1.
+    static constexpr int DQ = (EW <= 5) ? 2 : 1;
+    static constexpr int SCAP = 32 + 32 * QUAD * DQ;   // stack entries per warp: at most 31 left by the last drain + DQ quads
+    static constexpr int PLANE_BYTES = SCAP * 16;      // plane 0 (and every non-compact plane): 16 bytes per entry
     static constexpr bool COMPACT1 = (EW == 5);        // EW == 6: measured slower (sparse 64-bit stores hardly conflict; the extra address costs an issue slot per step)
     static constexpr int P1SHIFT = EW == 5 ? 2 : 1;
     static constexpr int STACK_BYTES = COMPACT1 ? SCAP * 16 + SCAP * 4 * (EW - 4) : PLANES * SCAP * 16;   // per warp
@@ -401,9 +404,6 @@ __device__ __forceinline__ void sts_v1_clr(uint32_t addr, uint32_t a, uint32_t w
 #ifndef PAIRINGS_SLOT_VARIANT
 #define PAIRINGS_SLOT_VARIANT 0
 #endif
-#ifndef PAIRINGS_TOP_VARIANT
-#define PAIRINGS_TOP_VARIANT 1
-#endif
 __device__ __forceinline__ void add16_clr(uint32_t& slot, uint32_t word, uint32_t bit) {
     asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.eq.u32 p, t, 0;\n\t@p add.u32 %0, %0, 16;\n\t}"
                  : "+r"(slot) : "r"(word), "r"(bit));
@@ -469,9 +469,15 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t k1, uint32_t
     } else {
         static_for<0, PL>([&](auto pc) {
             PAIRINGS_IC(pl, pc);
-            lds_v4(addr + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
+            lds_v4(addr + pl * L::PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
         });
     }
+#ifdef PAIRINGS_EXP_NODRAIN
+    { uint32_t x = 0;
+#pragma unroll
+      for (int i = 0; i < NR; i++) x ^= e[i];
+      acc[0] += x; return; }
+#endif
     uint32_t w[NR];
     static_for<0, NR>([&](auto rc) {                                              // bytes -> two's complement Q
         PAIRINGS_IC(r, rc);
@@ -624,12 +630,17 @@ struct Walker {
         // warp totals by REDUX (a byte sum is at most 128: no carry between fields): provably warp-uniform, which the
         // stack pointer and every drain loop inherit — the compiler then knows the warp stays converged
         tot[0] = __reduce_add_sync(0xffffffffu, c0); tot[1] = __reduce_add_sync(0xffffffffu, c1);
+        if constexpr (L::DQ == 2) ex[1] += tot[0];     // quads 2j and 2j+1 are pushed from the same stack pointer: 124 + 128 < 256
         nzc += (uint32_t)__popc(nzm);
     }
 
     template <int S>
     __device__ __forceinline__ void push_if_nonzero() {
         constexpr uint32_t bit = 1u << S;
+#ifdef PAIRINGS_EXP_NOSTORE
+        if constexpr (S % QUAD != QUAD - 1) add16_clr(slot, ZM, bit);
+        return;
+#endif
 #if PAIRINGS_SLOT_VARIANT == 1
         // the slot of the lane's next non-zero step goes to ANOTHER register, computed before the stores: an in-place
         // add would have to wait until the (variable-latency) stores have read their address register
@@ -648,9 +659,9 @@ struct Walker {
             static_for<0, L::PLANES>([&](auto pc) {
                 PAIRINGS_IC(pl, pc);
                 constexpr int words = (EW - 4 * pl) >= 4 ? 4 : (EW - 4 * pl);
-                if constexpr (words >= 3) sts_v4_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
-                else if constexpr (words == 2) sts_v2_clr(slot + pl * PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
-                else sts_v1_clr(slot + pl * PLANE_BYTES, e[4 * pl], ZM, bit);
+                if constexpr (words >= 3) sts_v4_clr(slot + pl * L::PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3], ZM, bit);
+                else if constexpr (words == 2) sts_v2_clr(slot + pl * L::PLANE_BYTES, e[4 * pl], e[4 * pl + 1], ZM, bit);
+                else sts_v1_clr(slot + pl * L::PLANE_BYTES, e[4 * pl], ZM, bit);
             });
         }
 #if PAIRINGS_SLOT_VARIANT == 1
@@ -683,22 +694,19 @@ struct Walker {
     template <int QI>
     __device__ __forceinline__ void quad() {
         constexpr uint32_t sel16 = 16u << (8 * (QI >> 1));                 // 16 * byte (QI >> 1) of word (QI & 1)
-#if PAIRINGS_TOP_VARIANT == 0
-        slot = __dp4a(ex[QI & 1], sel16, top);
-#else
-        slot = __dp4a(ex[QI & 1], sel16, 0u) + top;                        // top is warp-uniform: [R + UR] addressing
-#endif
+        slot = __dp4a(ex[QI & 1], sel16, 0u) + top;                        // top is warp-uniform (uniform datapath)
         static_for<QUAD * QI, QUAD * QI + QUAD>([&](auto sc) {
             PAIRINGS_IC(S, sc);
             push_if_nonzero<S>();
             if constexpr (S + 1 < BLK) inner_flip<zbits(S), ctz_c(S + 1)>();
         });
-#if PAIRINGS_TOP_VARIANT == 0
-        top = __dp4a(tot[QI & 1], sel16, top);
-#else
         constexpr int sh = 8 * (QI >> 1);                                  // uniform datapath: shift, mask, add
-        if constexpr (sh >= 4) top += (tot[QI & 1] >> (sh - 4)) & 0xFF0u; else top += (tot[QI & 1] << 4) & 0xFF0u;
-#endif
+        if constexpr (L::DQ == 1) {
+            if constexpr (sh >= 4) top += (tot[QI & 1] >> (sh - 4)) & 0xFF0u; else top += (tot[QI & 1] << 4) & 0xFF0u;
+        } else if constexpr (QI & 1) {                                     // both quads of the pair at once
+            if constexpr (sh >= 4) top += ((tot[0] >> (sh - 4)) & 0xFF0u) + ((tot[1] >> (sh - 4)) & 0xFF0u);
+            else top += ((tot[0] << 4) & 0xFF0u) + ((tot[1] << 4) & 0xFF0u);
+        }
     }
 
     // flip of inner bit bi in inner state ZB: dQ = -x_j * C[bi] + K  (row a3; K = inner neighbours, folded)
@@ -816,7 +824,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     const uint32_t warp_u = __reduce_min_sync(0xffffffffu, (unsigned)warp);          // the same value, known to be warp-uniform
     wk.top = stacks + warp_u * (uint32_t)L::STACK_BYTES;
     wk.lim = wk.top + 32u * 16u;
-    wk.k1 = wk.top + (uint32_t)(SCAP * 16) - (wk.top >> L::P1SHIFT);     // plane 1 starts behind plane 0
+    wk.k1 = wk.top + (uint32_t)L::PLANE_BYTES - (wk.top >> L::P1SHIFT);     // plane 1 starts behind plane 0
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
     unsigned long long nz = 0;
@@ -828,14 +836,14 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
         const uint64_t q = sub * per_block + (uint64_t)rd * blockDim.x + threadIdx.x;
         wk.init_prefix(chunk_base | (q << g));
         wk.nzc = 0;
-        // One inner block = BLK unrolled steps from inner state 0, a drain check every QUAD steps.
+        // One inner block = BLK unrolled steps from inner state 0, a drain check every DQ quads.
 #pragma unroll 1
         for (uint32_t u = 0; u < nblk; u++) {
             wk.zero_mask();
             static_for<0, BLK / QUAD>([&](auto qc) {
                 PAIRINGS_IC(QI, qc);
                 wk.template quad<QI>();
-                wk.drain_full();
+                if constexpr (QI % L::DQ == L::DQ - 1) wk.drain_full();
             });
             if (u + 1 < nblk) wk.block_end(H + (__ffs((int)(u + 1)) - 1));      // Gray order over the outer bits
         }
