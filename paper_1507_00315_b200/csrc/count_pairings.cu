@@ -355,12 +355,13 @@ int count_pairings_host(int kind, int n, int chunk_bits, uint64_t chunk_begin, u
     return PAIRINGS_OK;
 }
 
-int pairings_run_slice(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
-                       uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
-                       void* stream, const pairings_launch_opts* opts, unsigned flags,
-                       uint64_t slice_begin, uint64_t slice_end,
-                       uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
-                       uint64_t* duplicate_mismatches_out) {
+// the host driver; apply_symmetry: double the complete x_2 = +1 half (pairings_run_ex) or leave the raw sum (a slice)
+static int run_impl(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                    uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                    void* stream, const pairings_launch_opts* opts, unsigned flags,
+                    uint64_t slice_begin, uint64_t slice_end, bool apply_symmetry,
+                    uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                    uint64_t* duplicate_mismatches_out) {
     int rc = validate(kind, n, chunk_bits, slice_begin, slice_end, moduli, n_moduli, total_out); if (rc) return rc;
     if (!total_out || !chunks_done_out) return PAIRINGS_ENULL;
     if (chunks_per_call == 0) return PAIRINGS_EINVAL_CHUNK;
@@ -475,7 +476,7 @@ int pairings_run_slice(int kind, int n, int chunk_bits, const uint32_t* moduli, 
         *chunks_done_out += e - b;
         calls++;
     }
-    if (whole && *chunks_done_out == needed && multiplier == 2) {       // complete: H = 2 * (x_2 = +1 half)
+    if (apply_symmetry && whole && *chunks_done_out == needed && multiplier == 2) {       // complete: H = 2 * (x_2 = +1 half)
         rc = pairings_sum_rows(total_out, 1, moduli, n_moduli, total_out); if (rc) return rc;
     }
     return PAIRINGS_OK;
@@ -488,8 +489,18 @@ int pairings_run_ex(int kind, int n, int chunk_bits, const uint32_t* moduli, int
                     uint64_t* duplicate_mismatches_out) {
     int rc = check_kind_n(kind, n); if (rc) return rc;
     rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
-    return pairings_run_slice(kind, n, chunk_bits, moduli, n_moduli, chunks_per_call, journal_path, max_calls, stream, opts,
-                              flags, 0, 1ULL << chunk_bits, total_out, chunks_done_out, chunks_needed_out, duplicate_mismatches_out);
+    return run_impl(kind, n, chunk_bits, moduli, n_moduli, chunks_per_call, journal_path, max_calls, stream, opts,
+                    flags, 0, 1ULL << chunk_bits, true, total_out, chunks_done_out, chunks_needed_out, duplicate_mismatches_out);
+}
+
+int pairings_run_slice(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
+                       uint64_t chunks_per_call, const char* journal_path, int64_t max_calls,
+                       void* stream, const pairings_launch_opts* opts, unsigned flags,
+                       uint64_t slice_begin, uint64_t slice_end,
+                       uint32_t* total_out, uint64_t* chunks_done_out, uint64_t* chunks_needed_out,
+                       uint64_t* duplicate_mismatches_out) {
+    return run_impl(kind, n, chunk_bits, moduli, n_moduli, chunks_per_call, journal_path, max_calls, stream, opts,
+                    flags, slice_begin, slice_end, false, total_out, chunks_done_out, chunks_needed_out, duplicate_mismatches_out);
 }
 
 int pairings_run(int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,

@@ -92,6 +92,7 @@ __global__ void __launch_bounds__(PT_THREADS) pt_kernel(const PtParams p) {
             // ---- step 2: one move per level.  A move is evaluated from loads only (the four affected bins and
             // the old position), so the moves of two levels — different configurations — are evaluated together
             // and their dependent load chains overlap; shared memory is written only when a move is accepted.
+            // (Four levels at a time measured no faster: 8.3e10 against 8.5-8.7e10 moves/s.)
             struct Move { int slot, k, d, a0, a1, dE, j; };
             auto evaluate = [&](int j) -> Move {
                 Move m; m.j = j;

@@ -355,6 +355,21 @@ def test_slices_of_two_jobs_merge_to_the_count(tmp_path, paper_counts):
     assert cli.main(["L", "12", "--chunk-bits", "6", "--merge"] + js) == 0
 
 
+@pytest.mark.parametrize("extra", [[], ["--lemma24"], ["--lemma24", "--duplicate", "--audit"], ["--lemma24", "--rank", "0", "--world", "1"]])
+def test_command_line_prints_the_papers_count(extra, capsys):
+    import json
+    from paper_1507_00315_b200 import __main__ as cli
+    assert cli.main(["S", "16", "--json"] + extra) == 0
+    out = json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert (out["identified"], out["distinct"]) == (700078384, 1400156768)          # PAPER.md:352 (Table 7)
+    assert out["chunks_done"] == out["chunks_needed"] == (out["chunks"] // 2 if extra else out["chunks"])
+    # a whole run through the slice driver leaves the symmetry factor to the caller: raw sum = half of H
+    moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(S, 16) + 1)
+    raw, done, needed = pb.pairings_run_slice(S, 16, 8, moduli, 64, 0, 256, None, 0, 0, None, pb.RUN_LEMMA24)
+    full, fdone, fneeded = pb.pairings_run_ex(S, 16, 8, moduli, 64, None, 0, 0, None, pb.RUN_LEMMA24)
+    assert done == needed == fdone == fneeded == 128 and pb.pairings_sum_rows([raw], moduli, raw) == full
+
+
 @pytest.mark.parametrize("kind,n,C", [(L, 12, 6), (S, 13, 8), (L, 16, 10)])
 def test_generic_kernel_audits_the_fast_kernel(kind, n, C, paper_counts):
     moduli = pb.pairings_default_moduli(pb.pairings_bound_moduli(kind, n) + 1)

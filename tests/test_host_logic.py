@@ -373,3 +373,15 @@ def test_run_ex_without_pairings_needs_no_gpu():
     assert pb.pairings_reconstruct(pb.SKOLEM, 10, moduli, total) == (0, 0)
     with pytest.raises(pb.PairingsError):
         pb.pairings_run_ex(pb.SKOLEM, 10, 8, moduli, 64, None, 0, 0, None, 8)      # unknown flag
+
+
+def test_pt_draw_counter_must_not_wrap():
+    # the draw counter ((r (T+1) + tt) M + j) S + slot must stay below 2^64, else two replicas would share a random stream
+    # (the oracle wraps the same way, so parity could not show it): refused before anything is launched
+    betas = [0.0] + [0.5 * i for i in range(1, 32)]
+    with pytest.raises(pb.PairingsError) as ei:
+        pb.pairings_pt_run(pb.SKOLEM, 32, betas, 0, 1 << 30, 1 << 25, 0, 1, 0, 0, 0, 0)       # 2^30 * 2^25 * 32 * 32 = 2^65
+    assert ei.value.code == -10
+    with pytest.raises(pb.PairingsError) as ei:
+        pb.pairings_pt_run(pb.SKOLEM, 12, betas[:12], 0, 1 << 30, 1 << 25, 0, 1, 0, 0, 0, 0)  # in range: next check is the NULL pointers
+    assert ei.value.code == -5
