@@ -560,6 +560,17 @@ def run_gpu(args):
                                        s12_estimate=est, exact=227968, rel_error=est / 227968 - 1))
             if ptres["cpu_oracle"]:
                 ptres["gpu_over_cpu_oracle"] = moves_s / ptres["cpu_oracle"]["value"]
+            try:                                        # yardstick: executed instruction slots per move x moves/s against the issue peak
+                with open(NCU_METRICS) as f:
+                    pm = json.load(f)["pt"]
+                ptres["roofline"] = dict(bound="alu", thread_instr_slots_per_move=pm["thread_instr_slots_per_move"],
+                                         issue_frac=pm["thread_instr_slots_per_move"] * moves_s / peak, issue_active_pct=pm["issue_active_pct"],
+                                         active_threads_per_warp_instr=pm["active_threads_per_warp_instr"], ncu_source=pm["source"],
+                                         work_model="per move: one 64-bit SplitMix draw for colour and position (+ one for the acceptance when dE > 0), "
+                                                    "5 shared loads (old position, 4 bins), 5 shared stores when accepted; per level and iteration one "
+                                                    "histogram atomic and one exchange test (+ draw when dE > 0)")
+            except (OSError, ValueError, KeyError):
+                pass
 
         cpu = cpu_baseline(kind, n) if not args.no_cpu and not args.profile_chunks else None
         par = ("every rank the whole pass x%d, residue sums cross-checked (PAPER.md:99); each sign vector counted once" if duplicate
