@@ -21,10 +21,12 @@
 //    vector of the flipped position from two de-interleaved copies (E: even index bits, O: odd) of
 //    the sign word with a multiply-spread (4 bits -> 4 bytes), and patches one byte of each C[b].
 //    Because g <= n-2, every left neighbour of a walked position exists: no boundary guards at all.
-//  * non-zero terms are compacted (row a4's divergence problem): ballot + popc prefix push the packed
-//    registers into a per-warp shared-memory ring (the sign of the term is read off the distance-n sum); whenever 32 entries are queued all lanes
-//    multiply one entry each (any lane may process any term of its warp: the sum is commutative and
-//    a warp never spans two chunks).
+//  * non-zero terms are compacted (row a4's divergence problem).  The zero mask of a lane's whole block is known before
+//    its first step, so the slots of all pushes are PLANNED at block start: nibble popcounts give the lane's number of
+//    non-zero steps per quad (4 steps), one scan over the lanes in byte fields gives its first slot in every quad, REDUX
+//    the warp totals.  Entries (the packed registers; the sign of the term is read off the distance-n sum) go to a
+//    per-warp stack in shared memory with predicated stores; whenever 32 entries are stacked all lanes multiply one
+//    entry each (any lane may process any term of its warp: the sum is commutative and a warp never spans two chunks).
 //  * row a5: the product is formed from dp4a "pair factors" (two sums per LOP3 + IDP.4A), G exact
 //    signed group products (< 2^31 each), a signed multi-word product, added into a W-word
 //    two's-complement accumulator.  The reduction modulo the primes happens ONCE per thread (32-bit
@@ -159,7 +161,7 @@ struct Lay {
     // position exactly once, so #(x_i != x_{i+n}) = (n - P_n)/2 has the parity of #(x_i = -1).
     static constexpr int SIGN_SLOT = slot_of_d(NN);     // exists for both kinds (Skolem k = n, Langford k = n-1)
     static_assert(SIGN_SLOT >= 0, "distance n");
-    static constexpr int EW = NR;                       // ring entry words (the packed sums)
+    static constexpr int EW = NR;                       // stack entry words (the packed sums)
     static constexpr int PLANES = (EW + 3) / 4;         // planes per entry: plane 0 holds words 0..3 at a 16-byte stride
     // Plane 1 (words 4..) of a 5- or 6-word entry is COMPACT: 4 or 8 bytes per entry at that stride, so that the
     // 32-/64-bit accesses of a warp fall into distinct banks (at a 16-byte stride they are 4-/2-way conflicts —
@@ -305,7 +307,7 @@ static_assert(H == 5 && BLK == 32, "the zero-step masks are 32-bit words indexed
 static __device__ constexpr ZeroTables g_ztab = make_zero_tables();
 
 // ------------------------------------------------------------------------------------------------
-// ring entry -> signed multi-word term -> accumulator
+// stack entry -> signed multi-word term -> accumulator
 // ------------------------------------------------------------------------------------------------
 template <int W>
 __device__ __forceinline__ void acc_add_signed(uint32_t (&acc)[W], const uint32_t* x /* W words, already ^mask */, uint32_t mask) {
@@ -401,18 +403,9 @@ __device__ __forceinline__ void sts_v1_clr(uint32_t addr, uint32_t a, uint32_t w
                  :: "r"(addr), "r"(a), "r"(word), "r"(bit) : "memory");
 }
 // slot += 16 iff (word & bit) == 0 — the same predicate as the stores of that step
-#ifndef PAIRINGS_SLOT_VARIANT
-#define PAIRINGS_SLOT_VARIANT 0
-#endif
 __device__ __forceinline__ void add16_clr(uint32_t& slot, uint32_t word, uint32_t bit) {
     asm volatile("{\n\t.reg .pred p;\n\t.reg .b32 t;\n\tand.b32 t, %1, %2;\n\tsetp.eq.u32 p, t, 0;\n\t@p add.u32 %0, %0, 16;\n\t}"
                  : "+r"(slot) : "r"(word), "r"(bit));
-}
-// slot + 16 iff bit S of word is clear, as plain arithmetic (the result can live in another register than slot)
-template <int S>
-__device__ __forceinline__ uint32_t next_slot(uint32_t slot, uint32_t word) {
-    const uint32_t t = (word & (1u << S)) ^ (1u << S);
-    if constexpr (S >= 4) return slot + (t >> (S - 4)); else return slot + (t << (4 - S));
 }
 // one Kogge-Stone step of an inclusive scan over the lanes, two words at a time (byte fields that cannot overflow)
 template <int D>
@@ -641,12 +634,6 @@ struct Walker {
         if constexpr (S % QUAD != QUAD - 1) add16_clr(slot, ZM, bit);
         return;
 #endif
-#if PAIRINGS_SLOT_VARIANT == 1
-        // the slot of the lane's next non-zero step goes to ANOTHER register, computed before the stores: an in-place
-        // add would have to wait until the (variable-latency) stores have read their address register
-        uint32_t nxt = slot;
-        if constexpr (S % QUAD != QUAD - 1) nxt = next_slot<S>(slot, ZM);
-#endif
         // entry words: Q[0..NR); plane p holds words 4p..4p+3 (predicated vector stores, no branch)
         if constexpr (L::COMPACT1) {
             sts_v4_clr(slot, Q[0], Q[1], Q[2], Q[3], ZM, bit);
@@ -664,11 +651,7 @@ struct Walker {
                 else sts_v1_clr(slot + pl * L::PLANE_BYTES, e[4 * pl], ZM, bit);
             });
         }
-#if PAIRINGS_SLOT_VARIANT == 1
-        slot = nxt;
-#else
         if constexpr (S % QUAD != QUAD - 1) add16_clr(slot, ZM, bit);
-#endif
     }
 
     __device__ __forceinline__ void drain_full() {
@@ -788,7 +771,7 @@ struct Walker {
 
 template <int KIND, int NN>
 #ifndef PAIRINGS_SWAR_MINB
-#define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM (the ring limits it to 3 anyway): at most 85 registers; measured faster than 2 blocks without spills at n = 24
+#define PAIRINGS_SWAR_MINB 3   // 3 blocks of 256 threads per SM : at most 85 registers; measured faster than 2 blocks without spills at n = 24
 #endif
 #ifndef PAIRINGS_SWAR_BIG_N
 #define PAIRINGS_SWAR_BIG_N 25   // 7-8 packed registers, 35-40 neighbour registers: 2 blocks per SM without spills (measured: S(25) +4 %, L(27) +1.5 %, S(29) +7 % over 3 blocks with spills; n = 24 is 1 % faster with 3)

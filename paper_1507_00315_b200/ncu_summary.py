@@ -73,8 +73,9 @@ def bytes_of(value: str, unit: str) -> float:
 
 
 def source_breakdown(rep: str, terms: float, steps_per_block: int = 32):
-    """Executed warp-instructions per 32-step block, by how often an instruction runs per block (1 = the unrolled walk,
-    zero mask and slot plan; a fraction = the drain loops; rarely = outer flips, prefix init, tail) and by opcode."""
+    """Executed warp-instructions per 32-step block, by how often an instruction runs per block (exactly 1 = the
+    unrolled walk, zero mask and slot plan; another rate above 0.3 = the drain loops, whose rounds depend on the data;
+    rarely = outer flips, prefix init, tail) and by opcode."""
     rows = ncu_csv(rep, "source")
     hdr = rows[1]
     idx = {h: i for i, h in enumerate(hdr)}
@@ -88,7 +89,8 @@ def source_breakdown(rep: str, terms: float, steps_per_block: int = 32):
         src = r[idx["Source"]].strip().split()
         op = (src[1] if src[0].startswith("@") else src[0]).split(".")[0]
         ratio = ex / blocks
-        key = "once per block" if abs(ratio - 1) < 1e-9 else ("drain loops" if 0.3 < ratio < 1 else ("more than once per block" if ratio > 1 else "rarely"))
+        key = "once per block (walk, zero mask, slot plan)" if abs(ratio - 1) < 1e-9 else (
+            "loops inside a block (drain rounds)" if ratio > 0.3 else "rarely (outer flips, prefix init, tail)")
         sect[key][0] += 1
         sect[key][1] += ex * 32 / terms
         ops[op] += ex * 32 / terms
