@@ -36,7 +36,7 @@ struct KernelParams {
     int log2_bpc;         // log2(blocks per chunk)
     int n_moduli;
     uint32_t c80;         // 0x80808080, passed as data so that it stays in a register (SWAR drain: one LOP3 per masked operand)
-    uint32_t pad0;
+    uint32_t ztab_shared; // SWAR: 1 = every block copies the zero-step tables (24 KB) into shared memory (long-lived blocks)
     uint64_t chunk_begin;
     uint64_t n_chunks;
     uint32_t* out;        // DEVICE rows

@@ -305,6 +305,23 @@ PAIRINGS_HD ZeroTables make_zero_tables() {
 }
 static_assert(H == 5 && BLK == 32, "the zero-step masks are 32-bit words indexed by 5 pattern bits");
 static __device__ constexpr ZeroTables g_ztab = make_zero_tables();
+// The same masks in the layout of the per-block copy in shared memory (long-lived blocks, KernelParams::ztab_shared):
+// [shape][pattern 0..31][biased byte - ZB0], 64 words (256 bytes) per pattern, so that lanes which share a pattern — every
+// distance whose partners are walked bits — read consecutive words, and ONE dp4a forms 4 * byte + 256 * pattern.
+constexpr int ZB0 = 128 - ZR - 1;                        // first biased byte value with a table word (a 256-byte row holds 64)
+constexpr int ZSH_BYTES = 32 * 256;                      // bytes per shape
+constexpr int ZTAB_BYTES = ZSHAPES * ZSH_BYTES;
+static_assert(2 * ZR + 1 <= 63 && ZB0 >= 0, "a pattern row of 64 words holds every biased byte value [128 - ZR, 128 + ZR]");
+struct alignas(16) ZeroTablesT { uint32_t t[ZSHAPES][32][64]; };
+PAIRINGS_HD ZeroTablesT make_zero_tables_t() {
+    const ZeroTables T = make_zero_tables();
+    ZeroTablesT U{};
+    for (int sh = 0; sh < ZSHAPES; sh++)
+        for (int pat = 0; pat < 32; pat++)
+            for (int row = 0; row <= 2 * ZR; row++) U.t[sh][pat][row + 1] = T.t[sh][row][pat];   // word w <-> biased byte ZB0 + w
+    return U;
+}
+static __device__ constexpr ZeroTablesT g_ztab_t = make_zero_tables_t();
 
 // ------------------------------------------------------------------------------------------------
 // stack entry -> signed multi-word term -> accumulator
@@ -578,6 +595,8 @@ struct Walker {
     uint32_t top;
     uint32_t lim;             // stack base + 32 entries: a full drain round is possible while top >= lim
     uint32_t k1;              // compact plane 1: address of an entry's words 4.. = (plane-0 address >> P1SHIFT) + k1
+    uint32_t ztab;            // shared address of the block's zero-step tables, minus 4 * ZB0 (the dp4a offset starts at the
+                              // byte value); 0 = no copy in shared memory: read the tables in global memory (short-lived blocks)
     uint32_t lane16;          // lane * 16
     uint32_t c80;             // 0x80808080 (KernelParams::c80)
     uint32_t Vo;              // outer sign word: bit i = index bit H + i (set <-> x = -1)
@@ -591,25 +610,41 @@ struct Walker {
     // Row a4 for the whole block: OR over the even-distance slots of the table masks (see ztab above).
     __device__ __forceinline__ void zero_mask() {
         uint32_t zm = 0;
-        static_for<0, L::n_even()>([&](auto sc) {
-            PAIRINGS_IC(s, sc);
-            constexpr int d = L::d_of_slot(s), sh = zshape_of_d(d);
-            static_assert(L::bound(s) <= ZR, "table rows");
-            const uint32_t u = __byte_perm(Q[s / 4], 0, 0x4440 + (s % 4));                 // biased byte Q + 128
-            uint32_t pat4;                                                                  // 4 * pattern (byte offset in the row)
-            if constexpr (d >= H + 2) pat4 = (Vo >> (d - H - 2)) & 0x7Cu;
-            else if constexpr (d >= H) pat4 = (Vo << (H + 2 - d)) & 0x7Cu;
-            else pat4 = (Vo << 2) & (((1u << d) - 1u) << 2);
-            // address = table(shape) + (u - 128 + ZR) * 128 + pat4: the tables are 128-byte aligned, so pat4 is OR-ed
-            // into the low word of the (biased) base and ONE wide multiply-add forms the 64-bit address
-            const uint64_t base = (uint64_t)(uintptr_t)(&g_ztab.t[sh][0][0]) + (uint64_t)(int64_t)((ZR - 128) * 128);
-            uint64_t addr;
-            asm("{\n\t.reg .b32 lo, hi;\n\t.reg .b64 bp;\n\tmov.b64 {lo, hi}, %2;\n\tor.b32 lo, lo, %3;\n\tmov.b64 bp, {lo, hi};\n\t"
-                "mad.wide.u32 %0, %1, 128, bp;\n\t}" : "=l"(addr) : "r"(u), "l"(base), "r"(pat4));
-            uint32_t mask;
-            asm("ld.global.nc.u32 %0, [%1];" : "=r"(mask) : "l"(addr));
-            zm |= mask;
-        });
+        if (ztab != 0) {                              // warp-uniform (kernel parameter): the block's copy in shared memory
+            static_for<0, L::n_even()>([&](auto sc) {
+                PAIRINGS_IC(s, sc);
+                constexpr int d = L::d_of_slot(s), sh = zshape_of_d(d);
+                static_assert(L::bound(s) <= ZR, "table rows");
+                uint32_t pat256;                                                            // 256 * pattern
+                if constexpr (d >= H + 8) pat256 = (Vo >> (d - H - 8)) & 0x1F00u;
+                else if constexpr (d >= H) pat256 = (Vo << (H + 8 - d)) & 0x1F00u;
+                else pat256 = (Vo << 8) & (((1u << d) - 1u) << 8);
+                // ONE dp4a: 4 * (biased byte of the slot) + 256 * pattern; the shape's base is an immediate of the load
+                const uint32_t off = __dp4a(Q[s / 4], 4u << (8 * (s % 4)), pat256);
+                uint32_t mask;
+                lds_v1(ztab + (uint32_t)(sh * ZSH_BYTES) + off, mask);
+                zm |= mask;
+            });
+        } else {                                      // short-lived blocks: the tables in global memory (L1-resident)
+            static_for<0, L::n_even()>([&](auto sc) {
+                PAIRINGS_IC(s, sc);
+                constexpr int d = L::d_of_slot(s), sh = zshape_of_d(d);
+                const uint32_t u = __byte_perm(Q[s / 4], 0, 0x4440 + (s % 4));             // biased byte Q + 128
+                uint32_t pat4;                                                              // 4 * pattern (byte offset in the row)
+                if constexpr (d >= H + 2) pat4 = (Vo >> (d - H - 2)) & 0x7Cu;
+                else if constexpr (d >= H) pat4 = (Vo << (H + 2 - d)) & 0x7Cu;
+                else pat4 = (Vo << 2) & (((1u << d) - 1u) << 2);
+                // address = table(shape) + (u - 128 + ZR) * 128 + pat4: the tables are 128-byte aligned, so pat4 is OR-ed
+                // into the low word of the (biased) base and ONE wide multiply-add forms the 64-bit address
+                const uint64_t base = (uint64_t)(uintptr_t)(&g_ztab.t[sh][0][0]) + (uint64_t)(int64_t)((ZR - 128) * 128);
+                uint64_t addr;
+                asm("{\n\t.reg .b32 lo, hi;\n\t.reg .b64 bp;\n\tmov.b64 {lo, hi}, %2;\n\tor.b32 lo, lo, %3;\n\tmov.b64 bp, {lo, hi};\n\t"
+                    "mad.wide.u32 %0, %1, 128, bp;\n\t}" : "=l"(addr) : "r"(u), "l"(base), "r"(pat4));
+                uint32_t mask;
+                asm("ld.global.nc.u32 %0, [%1];" : "=r"(mask) : "l"(addr));
+                zm |= mask;
+            });
+        }
         ZM = zm;
         // ---- slot plan: per-lane counts of the non-zero steps of each quad (nibble popcounts of ~ZM), then an
         // inclusive scan over the lanes in byte fields (a field is at most 4 * 32 = 128)
@@ -784,13 +819,21 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     using L = Lay<KIND, NN>;
     using Wk = Walker<KIND, NN>;
     constexpr int N = L::N, B = N - 1, W = L::W;
-    extern __shared__ uint32_t smem[];
+    extern __shared__ __align__(16) uint32_t smem[];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    // dynamic shared memory (16-byte aligned): [stacks: warps x STACK_BYTES][reduction scratch]
-    const uint32_t stacks = (uint32_t)__cvta_generic_to_shared(smem);
+    // dynamic shared memory (16-byte aligned): [zero-step tables][stacks: warps x STACK_BYTES][reduction scratch]
+    const uint32_t smem0 = (uint32_t)__cvta_generic_to_shared(smem);
+    const uint32_t ztab_bytes = kp.ztab_shared ? (uint32_t)ZTAB_BYTES : 0u;
+    const uint32_t stacks = smem0 + ztab_bytes;
+    if (kp.ztab_shared) {                                                        // 24 KB, coalesced 16-byte copies
+        const uint4* src = reinterpret_cast<const uint4*>(&g_ztab_t.t[0][0][0]);
+        uint4* dst = reinterpret_cast<uint4*>(smem);
+        for (int i = threadIdx.x; i < ZTAB_BYTES / 16; i += blockDim.x) dst[i] = __ldg(src + i);
+        __syncthreads();
+    }
     const uint32_t stack_bytes = (blockDim.x >> 5) * (uint32_t)L::STACK_BYTES;
     unsigned long long* red = reinterpret_cast<unsigned long long*>(
-        reinterpret_cast<unsigned char*>(smem) + stack_bytes);                                    // 8 * 16 uint64
+        reinterpret_cast<unsigned char*>(smem) + ztab_bytes + stack_bytes);                       // 8 * 16 uint64
 
     const int C = kp.chunk_bits, g = kp.gray_bits;
     const uint64_t chunk_local = (uint64_t)blockIdx.x >> kp.log2_bpc;
@@ -807,6 +850,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     const uint32_t warp_u = __reduce_min_sync(0xffffffffu, (unsigned)warp);          // the same value, known to be warp-uniform
     wk.top = stacks + warp_u * (uint32_t)L::STACK_BYTES;
     wk.lim = wk.top + 32u * 16u;
+    wk.ztab = kp.ztab_shared ? smem0 - (uint32_t)(4 * ZB0) : 0u;
     wk.k1 = wk.top + (uint32_t)L::PLANE_BYTES - (wk.top >> L::P1SHIFT);     // plane 1 starts behind plane 0
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
@@ -860,7 +904,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
 template <int KIND, int NN>
 int launch(const KernelParams& kp, int block_threads, unsigned grid, void* stream) {
     using L = Lay<KIND, NN>;
-    const size_t smem = (size_t)(block_threads / 32) * L::STACK_BYTES
+    const size_t smem = (size_t)(kp.ztab_shared ? ZTAB_BYTES : 0) + (size_t)(block_threads / 32) * L::STACK_BYTES
                       + (size_t)(8 * PAIRINGS_MAX_MODULI * 2) * sizeof(uint32_t);
     cudaError_t e = cudaFuncSetAttribute(swar_kernel<KIND, NN>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return (int)e;
