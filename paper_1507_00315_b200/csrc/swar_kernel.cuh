@@ -306,19 +306,22 @@ PAIRINGS_HD ZeroTables make_zero_tables() {
 static_assert(H == 5 && BLK == 32, "the zero-step masks are 32-bit words indexed by 5 pattern bits");
 static __device__ constexpr ZeroTables g_ztab = make_zero_tables();
 // The same masks in the layout of the per-block copy in shared memory (long-lived blocks, KernelParams::ztab_shared):
-// [shape][pattern 0..31][biased byte - ZB0], 64 words (256 bytes) per pattern, so that lanes which share a pattern — every
-// distance whose partners are walked bits — read consecutive words, and ONE dp4a forms 4 * byte + 256 * pattern.
-constexpr int ZB0 = 128 - ZR - 1;                        // first biased byte value with a table word (a 256-byte row holds 64)
-constexpr int ZSH_BYTES = 32 * 256;                      // bytes per shape
+// [shape][biased byte - ZB0][pattern 0..31] with rows of 33 words (132 bytes), so that the bank of a word is
+// (byte + pattern) mod 32: lanes that share a pattern — every distance whose partners are walked bits — and differ in
+// the byte, and lanes that share the byte and differ in the pattern, all hit different banks.  ONE dp4a forms
+// 132 * byte + 4 * pattern.
+constexpr int ZB0 = 128 - ZR - 1;                        // first biased byte value with a table row (64 rows)
+constexpr int ZROW_BYTES = 132;                          // 32 patterns + one word of padding
+constexpr int ZSH_BYTES = 64 * ZROW_BYTES;               // bytes per shape
 constexpr int ZTAB_BYTES = ZSHAPES * ZSH_BYTES;
-static_assert(2 * ZR + 1 <= 63 && ZB0 >= 0, "a pattern row of 64 words holds every biased byte value [128 - ZR, 128 + ZR]");
-struct alignas(16) ZeroTablesT { uint32_t t[ZSHAPES][32][64]; };
+static_assert(2 * ZR + 1 <= 63 && ZB0 >= 0 && ZTAB_BYTES % 16 == 0 && ZROW_BYTES < 256, "64 rows hold every biased byte value [128 - ZR, 128 + ZR]");
+struct alignas(16) ZeroTablesT { uint32_t t[ZSHAPES][64][ZROW_BYTES / 4]; };
 PAIRINGS_HD ZeroTablesT make_zero_tables_t() {
     const ZeroTables T = make_zero_tables();
     ZeroTablesT U{};
     for (int sh = 0; sh < ZSHAPES; sh++)
         for (int pat = 0; pat < 32; pat++)
-            for (int row = 0; row <= 2 * ZR; row++) U.t[sh][pat][row + 1] = T.t[sh][row][pat];   // word w <-> biased byte ZB0 + w
+            for (int row = 0; row <= 2 * ZR; row++) U.t[sh][row + 1][pat] = T.t[sh][row][pat];   // row w <-> biased byte ZB0 + w
     return U;
 }
 static __device__ constexpr ZeroTablesT g_ztab_t = make_zero_tables_t();
@@ -595,7 +598,7 @@ struct Walker {
     uint32_t top;
     uint32_t lim;             // stack base + 32 entries: a full drain round is possible while top >= lim
     uint32_t k1;              // compact plane 1: address of an entry's words 4.. = (plane-0 address >> P1SHIFT) + k1
-    uint32_t ztab;            // shared address of the block's zero-step tables, minus 4 * ZB0 (the dp4a offset starts at the
+    uint32_t ztab;            // shared address of the block's zero-step tables, minus ZROW_BYTES * ZB0 (the dp4a offset starts at the
                               // byte value); 0 = no copy in shared memory: read the tables in global memory (short-lived blocks)
     uint32_t lane16;          // lane * 16
     uint32_t c80;             // 0x80808080 (KernelParams::c80)
@@ -615,12 +618,12 @@ struct Walker {
                 PAIRINGS_IC(s, sc);
                 constexpr int d = L::d_of_slot(s), sh = zshape_of_d(d);
                 static_assert(L::bound(s) <= ZR, "table rows");
-                uint32_t pat256;                                                            // 256 * pattern
-                if constexpr (d >= H + 8) pat256 = (Vo >> (d - H - 8)) & 0x1F00u;
-                else if constexpr (d >= H) pat256 = (Vo << (H + 8 - d)) & 0x1F00u;
-                else pat256 = (Vo << 8) & (((1u << d) - 1u) << 8);
-                // ONE dp4a: 4 * (biased byte of the slot) + 256 * pattern; the shape's base is an immediate of the load
-                const uint32_t off = __dp4a(Q[s / 4], 4u << (8 * (s % 4)), pat256);
+                uint32_t pat4;                                                              // 4 * pattern
+                if constexpr (d >= H + 2) pat4 = (Vo >> (d - H - 2)) & 0x7Cu;
+                else if constexpr (d >= H) pat4 = (Vo << (H + 2 - d)) & 0x7Cu;
+                else pat4 = (Vo << 2) & (((1u << d) - 1u) << 2);
+                // ONE dp4a: 132 * (biased byte of the slot) + 4 * pattern; the shape's base is an immediate of the load
+                const uint32_t off = __dp4a(Q[s / 4], (uint32_t)ZROW_BYTES << (8 * (s % 4)), pat4);
                 uint32_t mask;
                 lds_v1(ztab + (uint32_t)(sh * ZSH_BYTES) + off, mask);
                 zm |= mask;
@@ -850,7 +853,7 @@ swar_kernel(const __grid_constant__ KernelParams kp) {
     const uint32_t warp_u = __reduce_min_sync(0xffffffffu, (unsigned)warp);          // the same value, known to be warp-uniform
     wk.top = stacks + warp_u * (uint32_t)L::STACK_BYTES;
     wk.lim = wk.top + 32u * 16u;
-    wk.ztab = kp.ztab_shared ? smem0 - (uint32_t)(4 * ZB0) : 0u;
+    wk.ztab = kp.ztab_shared ? smem0 - (uint32_t)(ZROW_BYTES * ZB0) : 0u;
     wk.k1 = wk.top + (uint32_t)L::PLANE_BYTES - (wk.top >> L::P1SHIFT);     // plane 1 starts behind plane 0
 #pragma unroll
     for (int i = 0; i < W; i++) wk.acc[i] = 0;
