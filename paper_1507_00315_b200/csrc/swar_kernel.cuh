@@ -48,6 +48,9 @@ namespace swar {
 
 constexpr int H = PAIRINGS_SWAR_H;              // unrolled inner Gray bits
 constexpr int BLK = 1 << H;       // steps per unrolled block
+#ifndef PAIRINGS_DRAIN2_MAXEW
+#define PAIRINGS_DRAIN2_MAXEW 5   // larger entries have 8 drain sites per block: a second copy of the product there outgrows the instruction cache (S(24) -13 %)
+#endif
 constexpr int QUAD = 4;           // steps per slot allocation
 static_assert(31 * QUAD + 32 * QUAD <= 255, "per-quad lane prefixes (<= 31 * QUAD) are scanned in byte fields, and a warp total (<= 32 * QUAD) may be added to one");
 
@@ -693,6 +696,15 @@ struct Walker {
     }
 
     __device__ __forceinline__ void drain_full() {
+        if constexpr (L::EW <= PAIRINGS_DRAIN2_MAXEW) {
+            while (top >= lim + 32u * 16u) {                   // two rounds at once: half the loop overhead, the loads overlap
+                top -= 64u * 16u;
+                __syncwarp();
+                drain_entry<KIND, NN>(top + lane16, k1, acc, c80);
+                drain_entry<KIND, NN>(top + 32u * 16u + lane16, k1, acc, c80);
+                __syncwarp();
+            }
+        }
         while (top >= lim) {                                   // warp-uniform
             top -= 32u * 16u;
             __syncwarp();
