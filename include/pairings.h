@@ -52,7 +52,8 @@ enum {
     PAIRINGS_EINEXACT = -8,       /* H not divisible by 2^{2n-1}, or D odd (reading A16: never truncate) */
     PAIRINGS_ERANGE = -9,         /* product of the CRT moduli too small for the bound, or output buffer too small */
     PAIRINGS_EINVAL_OPTS = -10,   /* launch options not satisfiable for this (kind, n, chunk_bits) */
-    PAIRINGS_EJOURNAL = -11       /* journal file unreadable, or written for other parameters */
+    PAIRINGS_EJOURNAL = -11,      /* journal file unreadable, or written for other parameters */
+    PAIRINGS_ETOOBIG = -12        /* problem does not fit the fixed scratch area of a no-allocation entry point */
 };
 
 #define PAIRINGS_MAX_MODULI 16
@@ -309,6 +310,40 @@ int pairings_crt_signed(const uint32_t* moduli, int n_moduli, const uint32_t* re
 int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
                     uint64_t replica_begin, uint64_t replica_end, uint64_t iterations, uint64_t burn_in, uint64_t seed,
                     uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream);
+
+/* pairings_pt_run for callers that must not allocate device memory.
+ *
+ * Who needs this: pairings_pt_run takes its acceptance-threshold table (scratch the kernel reads, neither an input
+ * nor an output of the caller) from cudaMallocAsync and gives it back with cudaFreeAsync on every call.  Some
+ * programs cannot afford that.  A service that hands all of HBM to its own arena at start-up has nothing left for the
+ * driver to give out, so the allocation fails.  A loop with a latency budget cannot take an allocator call whose cost
+ * varies from microseconds to a device-wide synchronisation.  And code that runs where the CUDA allocator is simply
+ * off limits (a plug-in inside a host application that owns the memory budget) may only launch work.  This entry
+ * point runs the same kernel on the same arguments and produces the same counters, but its threshold table lives in
+ * a fixed array compiled into the library (`static __device__`, PAIRINGS_PT_STATIC_WORDS 64-bit words = 16 KiB).
+ * It calls neither cudaMalloc* nor cudaFree*, nor any library routine that allocates.  The price is 16 KiB of device
+ * memory on every GPU that loads the library, held until the process exits, whether or not this is ever called.
+ *
+ * Limit: the table holds n_levels * (2n + 3) words, and that must not exceed PAIRINGS_PT_STATIC_WORDS (2048); a
+ * larger request is refused with PAIRINGS_ETOOBIG before anything is enqueued (of the sizes pairings_pt_run takes,
+ * only n >= 31 with 31 or 32 levels are that large).  Everything else — arguments, counters that are ADDED to the
+ * caller's zeroed DEVICE arrays, the random streams, the other error codes, the one stream synchronisation while the
+ * table is staged from the host — is as documented for pairings_pt_run.
+ *
+ * Set-up: the first call on each device looks up the device address of the array (cudaGetSymbolAddress, with that
+ * device current) and remembers it per device; later calls on that device reuse it.  Make that first call before
+ * any stream capture begins, with the device you mean to use current.
+ *
+ * Sharing: there is ONE array per device and every call overwrites it.  Each call rewrites every word its kernel
+ * may read (including the never-accepted zero entries), so nothing left behind by an earlier call — a longer
+ * ladder, a larger n — can leak into a later one.  Calls enqueued on the same stream are ordered by the stream
+ * and are safe.  Two calls whose GPU work can overlap (different streams, or different host threads on different
+ * streams) race on the table: the first kernel may read the second call's thresholds.  Serialise them, or use
+ * pairings_pt_run for one of them. */
+#define PAIRINGS_PT_STATIC_WORDS 2048
+int pairings_pt_run_noalloc(int kind, int n, const double* betas, int n_levels,
+                            uint64_t replica_begin, uint64_t replica_end, uint64_t iterations, uint64_t burn_in, uint64_t seed,
+                            uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream);
 
 /* Ladder choice (exchange acceptance "no smaller than one half", as few levels as that allows).
  * Builds betas_out[0] = 0 < betas_out[1] < ... level by level: a pilot run (pilot_replicas x pilot_iterations, half

@@ -76,6 +76,7 @@ def lib():
         "pairings_reconstruct": (i, [i, i, u32p, i, u32p, cp, cp, ctypes.c_size_t]),
         "pairings_crt_signed": (i, [u32p, i, u32p, cp, ctypes.c_size_t]),
         "pairings_pt_run": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64, u64, u64, u64, u64, vp, vp, vp, vp]),
+        "pairings_pt_run_noalloc": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64, u64, u64, u64, u64, vp, vp, vp, vp]),
         "pairings_pt_ladder": (i, [i, i, ctypes.c_double, u64, u64, u64, ctypes.POINTER(ctypes.c_double), i, vp]),
         "pairings_pt_estimate": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64p, ctypes.POINTER(ctypes.c_double),
                                      ctypes.POINTER(ctypes.c_double)]),
@@ -318,6 +319,20 @@ def pairings_pt_run(kind, n, betas, replica_begin, replica_end, iterations, burn
     _check(lib().pairings_pt_run(kind, n, b, len(betas), replica_begin, replica_end, iterations, burn_in, seed,
                                  ctypes.c_void_p(hist_dev_ptr), ctypes.c_void_p(moves_dev_ptr),
                                  ctypes.c_void_p(swaps_dev_ptr), ctypes.c_void_p(stream)), "pairings_pt_run")
+
+
+def pairings_pt_run_noalloc(kind, n, betas, replica_begin, replica_end, iterations, burn_in, seed, hist_dev_ptr: int,
+                            moves_dev_ptr: int, swaps_dev_ptr: int, stream: int = 0):
+    """pairings_pt_run without any device allocation, for programs that cannot call cudaMalloc (all memory already
+    in their own arena, a latency budget, or a host application that forbids it): the kernel's threshold table sits
+    in a fixed 16 KiB array inside the library.  Same arguments and counters; n_levels * (2n + 3) must be <= 2048
+    (PairingsError with code -12 otherwise).  All calls on one device share that array, so calls whose GPU work may
+    overlap race; the first call on a device does a one-off address look-up and should precede any stream capture."""
+    b = (ctypes.c_double * len(betas))(*betas)
+    _check(lib().pairings_pt_run_noalloc(kind, n, b, len(betas), replica_begin, replica_end, iterations, burn_in, seed,
+                                         ctypes.c_void_p(hist_dev_ptr), ctypes.c_void_p(moves_dev_ptr),
+                                         ctypes.c_void_p(swaps_dev_ptr), ctypes.c_void_p(stream)),
+           "pairings_pt_run_noalloc")
 
 
 def pairings_pt_ladder(kind, n, target_exchange=0.55, pilot_replicas=256, pilot_iterations=1 << 14, seed=1,

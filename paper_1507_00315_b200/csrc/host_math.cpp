@@ -582,6 +582,7 @@ const char* pairings_strerror(int code) {
         case PAIRINGS_ERANGE: return "modulus product too small for the bound, or output buffer too small";
         case PAIRINGS_EINVAL_OPTS: return "launch options not satisfiable";
         case PAIRINGS_EJOURNAL: return "journal unreadable or written for other parameters";
+        case PAIRINGS_ETOOBIG: return "problem too large for the fixed scratch area of a no-allocation entry point";
         default: return "unknown error code";
     }
 }

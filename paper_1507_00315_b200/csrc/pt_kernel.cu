@@ -28,6 +28,7 @@
 
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 namespace pairings {
@@ -185,6 +186,31 @@ static int pt_check(int kind, int n, const double* betas, int n_levels) {
     return PAIRINGS_OK;
 }
 
+// ---- pairings_pt_run_noalloc: the threshold table in a fixed array of the library's own instead of cudaMallocAsync.
+// Every GPU that loads this library holds these 16 KiB until the process exits.  The name is usable as it stands only
+// in device code: on the host it is a stand-in symbol, not a device pointer — a kernel handed `pt_static_thr` itself
+// would fault (or quietly read host memory on systems where the GPU can reach it).  Host code therefore asks the
+// runtime for the real address, once per device with that device current, and passes that to the kernel.
+static __device__ __align__(256) unsigned long long pt_static_thr[PAIRINGS_PT_STATIC_WORDS];
+
+// Device address of pt_static_thr on the current device (looked up on the first call per device, then remembered).
+static int pt_static_address(uint64_t** out) {
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static uint64_t* known[MAX_DEV] = {};
+    int dev = -1;
+    (void)cudaGetLastError();
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev < MAX_DEV && known[dev]) { *out = known[dev]; return PAIRINGS_OK; }
+    void* ptr = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&ptr, pt_static_thr);
+    if (e != cudaSuccess || ptr == nullptr) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    if (dev < MAX_DEV) known[dev] = (uint64_t*)ptr;
+    *out = (uint64_t*)ptr;
+    return PAIRINGS_OK;
+}
+
 }  // namespace pairings
 
 using namespace pairings;
@@ -236,6 +262,61 @@ int pairings_pt_run(int kind, int n, const double* betas, int n_levels,
     }
     cudaError_t e2 = cudaFreeAsync(dthr, s);
     if (e != cudaSuccess || e2 != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
+    return PAIRINGS_OK;
+}
+
+// Same replicas, same kernel, same counters as pairings_pt_run, for callers that may not allocate on the device
+// (include/pairings.h says who and why).  No cudaMalloc*/cudaFree*, no std::vector: the table is built in a stack
+// array and staged into pt_static_thr, which every call on this device shares — see the header for the race rule.
+int pairings_pt_run_noalloc(int kind, int n, const double* betas, int n_levels,
+                            uint64_t replica_begin, uint64_t replica_end, uint64_t iterations, uint64_t burn_in, uint64_t seed,
+                            uint64_t* hist_dev, uint64_t* moves_dev, uint64_t* swaps_dev, void* stream) {
+    int rc = pt_check(kind, n, betas, n_levels); if (rc) return rc;
+    if (replica_begin > replica_end || iterations == 0 || iterations > (1ULL << 25) || burn_in >= iterations) return PAIRINGS_EINVAL_OPTS;
+    if (replica_end > (1ULL << 30)) return PAIRINGS_EINVAL_OPTS;
+    {   // the draw counter must not wrap (as in pairings_pt_run)
+        const unsigned __int128 span = (unsigned __int128)replica_end * (iterations + 1) * (unsigned)n_levels * (unsigned)(n > 3 ? n : 3);
+        if (span >> 64) return PAIRINGS_EINVAL_OPTS;
+    }
+    const int M = n_levels, N = 2 * n;
+    const size_t words = (size_t)M * 2 + (size_t)M * (size_t)(N + 1);          // move thresholds, then exchange thresholds
+    if (words > (size_t)PAIRINGS_PT_STATIC_WORDS) return PAIRINGS_ETOOBIG;     // refused before anything is enqueued
+    if (!hist_dev || !moves_dev || !swaps_dev) return PAIRINGS_ENULL;
+    if (replica_begin == replica_end) return PAIRINGS_OK;
+
+    // All `words` entries are written, also the ones no decision ever reads (dE = 0, the row above the last level):
+    // the array still holds the previous call's table and none of it may survive inside this call's extent.
+    uint64_t thr[PAIRINGS_PT_STATIC_WORDS];
+    for (size_t i = 0; i < words; i++) thr[i] = 0;
+    for (int j = 0; j < M; j++)
+        for (int dE = 1; dE <= 2; dE++) thr[(size_t)(j * 2 + dE - 1)] = pt_threshold(std::exp(-betas[j] * (double)dE));
+    for (int j = 0; j + 1 < M; j++)
+        for (int dE = 1; dE <= N; dE++)
+            thr[(size_t)(M * 2 + j * (N + 1) + dE)] = pt_threshold(std::exp(-(betas[j + 1] - betas[j]) * (double)dE));
+
+    uint64_t* table = nullptr;                                                 // DEVICE address of pt_static_thr
+    rc = pt_static_address(&table); if (rc) return rc;                         // first call on this device: the set-up
+
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(table, thr, words * sizeof(uint64_t), cudaMemcpyHostToDevice, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);                        // thr is a local: the copy must have left it
+    PtParams p; std::memset(&p, 0, sizeof p);
+    p.kind = kind; p.n = n; p.M = M;
+    p.replica_begin = replica_begin; p.replica_end = replica_end; p.iterations = iterations; p.burn_in = burn_in; p.seed = seed;
+    p.move_thr = table; p.swap_thr = table + M * 2;
+    p.hist = (unsigned long long*)hist_dev; p.moves = (unsigned long long*)moves_dev; p.swaps = (unsigned long long*)swaps_dev;
+    const bool nib = n <= 15;
+    const size_t occ_bytes = nib ? (size_t)(N + 2) / 2 : (size_t)(N + 1);
+    const size_t smem = (size_t)(M * (N + 1) + 2 * M) * sizeof(unsigned int)
+                      + (size_t)PT_THREADS * ((size_t)M * n + (size_t)M * occ_bytes + 2 * (size_t)M);
+    auto kernel = nib ? pt_kernel<true> : pt_kernel<false>;
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e == cudaSuccess) {
+        const uint64_t blocks = (replica_end - replica_begin + PT_THREADS - 1) / PT_THREADS;
+        kernel<<<(unsigned)blocks, PT_THREADS, smem, s>>>(p);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) { (void)cudaGetLastError(); return PAIRINGS_ECUDA; }
     return PAIRINGS_OK;
 }
 

@@ -35,7 +35,7 @@ def test_library_exports_every_declared_symbol(built):
 
 def test_strerror_and_build_info():
     assert pb.pairings_strerror(0) == "ok"
-    for code in range(-11, 0):
+    for code in range(-12, 0):
         assert pb.pairings_strerror(code) != "unknown error code"
     assert "sm_100a" in pb.pairings_build_info()
 
