@@ -190,6 +190,32 @@ int64_t pairings_journal_merge(const char* const* paths, int n_paths, const char
                                int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli,
                                uint32_t* total_out, uint64_t* chunks_covered_out);
 
+/* The mode of a job, in one place (host only).  `flags` are the PAIRINGS_RUN_* bits of pairings_run_ex (declared
+ * below; only PAIRINGS_RUN_LEMMA24 changes anything here).
+ *
+ * pairings_mode_chunks: *needed_out = the number of chunks a whole job evaluates in this mode, always the range
+ * [0, needed): 2^chunk_bits without the symmetry; with PAIRINGS_RUN_LEMMA24 and chunk_bits >= 1 the x_2 = +1 half
+ * [0, 2^(chunk_bits-1)) when the two halves are equal, 0 when they cancel (Lemma 2.4; the most
+ * significant chunk bit is x_2).  Returns the factor that turns the sum over those chunks into H: 1, 2 or 0 (H = 0),
+ * or a negative code.
+ *
+ * pairings_finish_total: the last step of a job whose rows were added up elsewhere (a slice run alone, merged
+ * journals).  If chunks_covered equals the mode's chunk count, total_inout (HOST, n_moduli residues of the raw row
+ * sum) is multiplied by that factor — the ONLY place outside pairings_run_ex where Lemma 2.4's doubling is applied —
+ * and 1 is returned: total_inout is H mod p_i, ready for pairings_reconstruct.  Fewer chunks: returns 0, total
+ * untouched.  More: PAIRINGS_EINVAL_CHUNK.
+ *
+ * pairings_journal_merge_mode: pairings_journal_merge for a given mode — additionally refuses (PAIRINGS_EJOURNAL) any
+ * range that reaches outside [0, needed), so that journals of jobs run without the symmetry, or a mix of ranges from
+ * both halves that merely adds up to the right length, cannot be doubled into a wrong count; *chunks_needed_out (may
+ * be NULL) = needed.  The sum is NOT finished: pass it with *chunks_covered_out to pairings_finish_total. */
+int pairings_mode_chunks(int kind, int n, int chunk_bits, unsigned flags, uint64_t* needed_out);
+int pairings_finish_total(int kind, int n, int chunk_bits, unsigned flags, uint64_t chunks_covered,
+                          const uint32_t* moduli, int n_moduli, uint32_t* total_inout);
+int64_t pairings_journal_merge_mode(const char* const* paths, int n_paths, const char* out_path,
+                                    int kind, int n, int chunk_bits, const uint32_t* moduli, int n_moduli, unsigned flags,
+                                    uint32_t* total_out, uint64_t* chunks_covered_out, uint64_t* chunks_needed_out);
+
 /* The duplicate-run protocol against silent GPU errors ("every GPU job was ran twice on separate GPUs.
  * The two results were then matched, if there was a mismatch the job was ran a third time to establish a match").
  * pairings_vote_rows compares n_words words (HOST): returns 0 if a == b, or if c (the third run, may be NULL) equals
@@ -237,9 +263,11 @@ int pairings_lemma24(int kind, int n);
  *
  * PAIRINGS_RUN_AUDIT: a cheap second opinion from an independent implementation — of every chunk range, the first
  * chunk and one seeded chunk are evaluated again by PAIRINGS_VARIANT_GENERIC (other kernel, other arithmetic: per-term
- * Montgomery residues instead of exact multi-word sums) and compared word by word; on a mismatch a third run of that
- * chunk (the fast kernel at another Gray-bit count) votes: if it sides with the fast kernel the range stands (the
- * mismatch is counted), otherwise the call fails with PAIRINGS_ECHECK.  Costs a few per cent. */
+ * Montgomery residues instead of exact multi-word sums) and compared word by word; on a mismatch the auditor itself
+ * runs that chunk once more at another Gray-bit count and decides: if this second generic run sides with the fast
+ * row, the auditor's first run was a transient fault and the range stands (the mismatch is counted); if the generic
+ * kernel reproduces its own row — so the fast kernel is wrong, however often it reproduces itself — or no two rows
+ * agree, the call fails with PAIRINGS_ECHECK.  The audited kernel never votes on itself.  Costs a few per cent. */
 enum { PAIRINGS_RUN_LEMMA24 = 1, PAIRINGS_RUN_DUPLICATE = 2, PAIRINGS_RUN_AUDIT = 4 };
 int pairings_run_ex(int kind, int n, int chunk_bits,
                     const uint32_t* moduli, int n_moduli,

@@ -10,7 +10,8 @@ from .api import (  # noqa: F401
     pairings_default_moduli, pairings_min_moduli, pairings_bound_moduli,
     pairings_partition, pairings_rank_range, pairings_sum_rows,
     pairings_journal_append, pairings_journal_load, pairings_run, pairings_run_ex, pairings_run_slice, pairings_lemma24,
-    RUN_LEMMA24, RUN_DUPLICATE, RUN_AUDIT, pairings_journal_merge, pairings_vote_rows, pairings_duplicate_vote,
+    RUN_LEMMA24, RUN_DUPLICATE, RUN_AUDIT, pairings_journal_merge, pairings_journal_merge_mode,
+    pairings_mode_chunks, pairings_finish_total, pairings_vote_rows, pairings_duplicate_vote,
     default_chunk_bits, default_chunks_per_call,
     pairings_reconstruct, pairings_crt_signed, pairings_strerror, pairings_build_info,
     pairings_pt_run, pairings_pt_run_noalloc, pairings_pt_estimate, pairings_pt_ladder,

@@ -74,33 +74,32 @@ def main(argv=None) -> int:
     moduli = api.pairings_default_moduli(m)
     C = a.chunk_bits if a.chunk_bits is not None else api.default_chunk_bits(n)
     per_call = a.chunks_per_call if a.chunks_per_call is not None else api.default_chunks_per_call(n, C)
-    lemma = bool(a.lemma24) and C >= 1
-    sym = api.pairings_lemma24(kind, n) if lemma else 1           # 1: halves equal, 0: halves cancel (H = 0)
-    job_chunks = (1 << C) if not lemma else ((1 << (C - 1)) if sym == 1 else 0)    # chunks this mode evaluates
     flags = (api.RUN_LEMMA24 if a.lemma24 else 0) | (api.RUN_DUPLICATE if a.duplicate else 0) | (api.RUN_AUDIT if a.audit else 0)
+    # chunks [0, job_chunks) are what this mode evaluates; Lemma 2.4's rule lives behind the ABI (pairings_mode_chunks,
+    # pairings_finish_total), the command line never applies a factor of its own
+    job_chunks, _factor = api.pairings_mode_chunks(kind, n, C, flags)
 
     if a.merge is not None:                                       # put the jobs' results together (host only)
         t0 = time.perf_counter()
         if job_chunks == 0:
             ranges, total, covered = 0, [0] * m, 0
         else:
-            ranges, total, covered = api.pairings_journal_merge(a.merge, kind, n, C, moduli, a.journal)
+            ranges, total, covered, _needed = api.pairings_journal_merge_mode(a.merge, kind, n, C, moduli, flags, a.journal)
         res = dict(kind=a.kind.upper(), n=n, chunk_bits=C, moduli=moduli, merged=list(a.merge), ranges=ranges,
                    chunks_done=covered, chunks_needed=job_chunks, lemma24=bool(a.lemma24), total_residues=total,
                    seconds=time.perf_counter() - t0)
-        if covered == job_chunks:
-            if lemma and sym == 1:                                # H = 2 x (the x_2 = +1 half)
-                total = api.pairings_sum_rows([total], moduli, total)
+        complete, total = api.pairings_finish_total(kind, n, C, flags, covered, moduli, total)
+        if complete:
             D, S = api.pairings_reconstruct(kind, n, moduli, total)
             res.update(distinct=D, identified=S, total_residues=total)
         if a.json:
             print(json.dumps(res))
-        elif covered == job_chunks:
+        elif complete:
             print("%s(%d): reflections identified %d, distinct %d  (%d journals, %d ranges)" %
                   (res["kind"], n, res["identified"], res["distinct"], len(a.merge), ranges))
         else:
             print("%s(%d): the journals cover %d of %d chunks; the count needs all of them" % (res["kind"], n, covered, job_chunks))
-        return 0 if covered == job_chunks else 3
+        return 0 if complete else 3
 
     if not 0 <= a.rank < a.world:
         ap.error("--rank must be in [0, --world)")
@@ -110,7 +109,7 @@ def main(argv=None) -> int:
     elif a.world == 1:
         sb, se = 0, job_chunks
     else:
-        sb, se = api.pairings_rank_range(C if not lemma else C - 1, a.rank, a.world)
+        sb, se = api.pairings_rank_range(job_chunks.bit_length() - 1, a.rank, a.world)     # job_chunks is a power of two
     ti = time.perf_counter()
     api.count_pairings_host(api.LANGFORD, 3, 0, 0, 1, moduli[:1])      # CUDA context + module load, outside the timing
     init_s = time.perf_counter() - ti
@@ -121,12 +120,15 @@ def main(argv=None) -> int:
                chunks=1 << C, slice=[sb, se], rank=a.rank, world=a.world, lemma24=bool(a.lemma24), duplicate=bool(a.duplicate),
                audit=bool(a.audit), duplicate_mismatches=api.pairings_run_slice.last_mismatches, seconds=dt, init_seconds=init_s,
                total_residues=total)
+    if res["duplicate_mismatches"]:                               # a vote was needed: the count stands, the hardware is suspect
+        sys.stderr.write("warning: %d chunk range(s) had disagreeing runs and were settled by a vote (PAPER.md:99); "
+                         "check this GPU\n" % res["duplicate_mismatches"])
     evaluated = needed << (2 * n - 1 - C)
     res.update(terms_evaluated=evaluated, terms_per_s=evaluated / dt if dt > 0 and done == needed else None)
-    whole = a.world == 1 and done == needed
+    whole = False
+    if a.world == 1:                                              # a slice run alone: finished like merged journals
+        whole, total = api.pairings_finish_total(kind, n, C, flags, done, moduli, total)
     if whole:
-        if lemma and sym == 1:
-            total = api.pairings_sum_rows([total], moduli, total)
         D, S = api.pairings_reconstruct(kind, n, moduli, total)
         res.update(distinct=D, identified=S, total_residues=total)
     if a.json:

@@ -70,6 +70,10 @@ def lib():
         "pairings_run_slice": (i, [i, i, i, u32p, i, u64, cp, ctypes.c_int64, vp, optp, ctypes.c_uint, u64, u64, u32p, u64p, u64p,
                                    u64p]),
         "pairings_journal_merge": (ctypes.c_int64, [ctypes.POINTER(cp), i, cp, i, i, i, u32p, i, u32p, u64p]),
+        "pairings_journal_merge_mode": (ctypes.c_int64, [ctypes.POINTER(cp), i, cp, i, i, i, u32p, i, ctypes.c_uint, u32p, u64p,
+                                                         u64p]),
+        "pairings_mode_chunks": (i, [i, i, i, ctypes.c_uint, u64p]),
+        "pairings_finish_total": (i, [i, i, i, ctypes.c_uint, u64, u32p, i, u32p]),
         "pairings_vote_rows": (i, [u32p, u32p, u32p, u64]),
         "pairings_duplicate_vote": (i, [EVAL_FN, vp, u64, u32p, ctypes.POINTER(i)]),
         "pairings_lemma24": (i, [i, i]),
@@ -275,6 +279,35 @@ def pairings_journal_merge(paths, kind, n, chunk_bits, moduli, out_path=None):
     return int(nr), [int(t[j]) for j in range(k)], int(cov.value)
 
 
+def pairings_journal_merge_mode(paths, kind, n, chunk_bits, moduli, flags: int = 0, out_path=None):
+    """pairings_journal_merge for a job mode (RUN_* flags): ranges outside the chunks that mode evaluates are refused.
+    Returns (ranges, raw total residues, chunks covered, chunks needed); finish with pairings_finish_total."""
+    arr = (ctypes.c_char_p * len(paths))(*[os.fsencode(p) for p in paths])
+    total = (ctypes.c_uint32 * len(moduli))()
+    cov, need = ctypes.c_uint64(0), ctypes.c_uint64(0)
+    nr = _check(lib().pairings_journal_merge_mode(arr, len(paths), os.fsencode(out_path) if out_path else None, kind, n,
+                                                  chunk_bits, _u32(moduli), len(moduli), flags, total, ctypes.byref(cov),
+                                                  ctypes.byref(need)), "pairings_journal_merge_mode")
+    return nr, [int(v) for v in total], int(cov.value), int(need.value)
+
+
+def pairings_mode_chunks(kind, n, chunk_bits, flags: int = 0):
+    """(chunks a whole job evaluates in this mode — always the range [0, needed) —, factor 1 / 2 / 0 that turns
+    their sum into H).  Lemma 2.4."""
+    need = ctypes.c_uint64(0)
+    f = _check(lib().pairings_mode_chunks(kind, n, chunk_bits, flags, ctypes.byref(need)), "pairings_mode_chunks")
+    return int(need.value), f
+
+
+def pairings_finish_total(kind, n, chunk_bits, flags, chunks_covered, moduli, total):
+    """(complete?, total): when chunks_covered is the mode's whole chunk count, `total` (raw row sum) times the
+    mode's factor = H mod p_i, ready for pairings_reconstruct; otherwise (False, total unchanged)."""
+    t = _u32(total)
+    rc = _check(lib().pairings_finish_total(kind, n, chunk_bits, flags, chunks_covered, _u32(moduli), len(moduli), t),
+                "pairings_finish_total")
+    return bool(rc), [int(v) for v in t]
+
+
 def pairings_vote_rows(a, b, c=None) -> int:
     """0: a stands, 1: b stands, 3: a != b and no third run given; raises PairingsError(ECHECK) if no two agree."""
     return _check(lib().pairings_vote_rows(_u32(a), _u32(b), _u32(c) if c is not None else None, len(a)),
@@ -282,18 +315,32 @@ def pairings_vote_rows(a, b, c=None) -> int:
 
 
 def pairings_duplicate_vote(evaluate, n_words: int):
-    """evaluate(attempt) -> list of n_words ints (or a negative error code).  Returns (rows, mismatch)."""
+    """evaluate(attempt) -> list of n_words ints (or a negative error code).  Returns (rows, mismatch).
+    An exception raised by evaluate, or a row of the wrong length, stops the vote (the C side sees PAIRINGS_ECHECK, so
+    two failed attempts can never 'agree' on unfilled rows) and is re-raised here."""
+    failure = []
+
     def thunk(_ctx, attempt, out):
-        r = evaluate(int(attempt))
-        if isinstance(r, int):
-            return r
-        for j, v in enumerate(r):
-            out[j] = v
-        return 0
+        try:                                      # ctypes would swallow the exception and hand 0 (= success) to C
+            r = evaluate(int(attempt))
+            if isinstance(r, int):
+                return r if r < 0 else -7         # a code is an error; 0 or positive without rows is one too
+            r = list(r)
+            if len(r) != n_words:
+                raise ValueError("evaluate(%d) returned %d words, expected %d" % (attempt, len(r), n_words))
+            for j, v in enumerate(r):
+                out[j] = v
+            return 0
+        except BaseException as exc:              # noqa: BLE001 — re-raised after the C call returns
+            failure.append(exc)
+            return -7
     cb = EVAL_FN(thunk)
     rows = (ctypes.c_uint32 * max(n_words, 1))()
     mm = ctypes.c_int(0)
-    _check(lib().pairings_duplicate_vote(cb, None, n_words, rows, ctypes.byref(mm)), "pairings_duplicate_vote")
+    rc = lib().pairings_duplicate_vote(cb, None, n_words, rows, ctypes.byref(mm))
+    if failure:
+        raise failure[0]
+    _check(rc, "pairings_duplicate_vote")
     return [int(rows[j]) for j in range(n_words)], int(mm.value)
 
 

@@ -376,14 +376,11 @@ static int run_impl(int kind, int n, int chunk_bits, const uint32_t* moduli, int
     // Lemma 2.4: negating the even positions maps the x_2 = +1 half of every
     // sum onto the x_2 = -1 half, term for term (up to the sign pairings_lemma24 reports).  The most
     // significant chunk bit is x_2, so the x_2 = +1 half is the chunk range [0, 2^{C-1}).
-    uint64_t needed = 1ULL << chunk_bits;
-    uint32_t multiplier = 1;
-    if ((flags & PAIRINGS_RUN_LEMMA24) && chunk_bits >= 1) {
-        const int sym = pairings_lemma24(kind, n);
-        if (sym < 0) return sym;
-        if (sym == 1) { needed >>= 1; multiplier = 2; }
-        else { needed = 0; multiplier = 0; }           // the two halves cancel: H = 0, nothing to evaluate
-    }
+    // pairings_mode_chunks (host_math.cpp) is the one statement of that rule: chunks [0, needed), factor 1, 2 or 0
+    // (the two halves cancel: H = 0, nothing to evaluate).
+    uint64_t needed = 0;
+    const int multiplier = pairings_mode_chunks(kind, n, chunk_bits, flags, &needed);
+    if (multiplier < 0) return multiplier;
     // a slice (one job of a chunk farm): only chunks of [slice_begin, slice_end) that this mode evaluates
     const uint64_t sb = std::min(slice_begin, needed), se = std::min(slice_end, needed);
     const bool whole = (sb == 0 && se == needed);
@@ -423,8 +420,9 @@ static int run_impl(int kind, int n, int chunk_bits, const uint32_t* moduli, int
         rows.resize((size_t)(e - b) * (size_t)n_moduli);
         // another launch geometry of the same kernel variant: the nearest admissible Gray-bit count (other thread <->
         // term mapping, other summation order); if none exists (tiny jobs) the same geometry again
-        auto rerun_other_geometry = [&](int first_dg, uint64_t rb, uint64_t re, uint32_t* dst) -> int {
-            Geometry geo; int rc2 = choose_geometry(kind, n, chunk_bits, re - rb, opts, &geo); if (rc2) return rc2;
+        auto rerun_other_geometry = [&](int first_dg, uint64_t rb, uint64_t re, uint32_t* dst,
+                                        const pairings_launch_opts* base) -> int {
+            Geometry geo; int rc2 = choose_geometry(kind, n, chunk_bits, re - rb, base, &geo); if (rc2) return rc2;
             pairings_launch_opts alt; std::memset(&alt, 0, sizeof alt);
             alt.variant = geo.variant;
             rc2 = PAIRINGS_EINVAL_OPTS;
@@ -432,7 +430,7 @@ static int run_impl(int kind, int n, int chunk_bits, const uint32_t* moduli, int
                 alt.gray_bits = geo.g - dg > 0 ? geo.g - dg : geo.g + dg;
                 rc2 = count_pairings_host(kind, n, chunk_bits, rb, re, moduli, n_moduli, dst, stream, &alt);
             }
-            if (rc2 == PAIRINGS_EINVAL_OPTS) rc2 = count_pairings_host(kind, n, chunk_bits, rb, re, moduli, n_moduli, dst, stream, opts);
+            if (rc2 == PAIRINGS_EINVAL_OPTS) rc2 = count_pairings_host(kind, n, chunk_bits, rb, re, moduli, n_moduli, dst, stream, base);
             return rc2;
         };
         if (flags & PAIRINGS_RUN_DUPLICATE) {
@@ -444,7 +442,7 @@ static int run_impl(int kind, int n, int chunk_bits, const uint32_t* moduli, int
             auto eval = [](void* c, int attempt, uint32_t* out) -> int {
                 Ctx* x = static_cast<Ctx*>(c);
                 if (attempt == 0) return count_pairings_host(x->kind, x->n, x->C, x->b, x->e, x->moduli, x->m, out, x->stream, x->opts);
-                return (*x->rerun)(attempt, x->b, x->e, out);
+                return (*x->rerun)(attempt, x->b, x->e, out, x->opts);
             };
             int mismatch = 0;
             rc = pairings_duplicate_vote(eval, &ctx, (uint64_t)rows.size(), rows.data(), &mismatch); if (rc) return rc;
@@ -465,7 +463,12 @@ static int run_impl(int kind, int n, int chunk_bits, const uint32_t* moduli, int
                 const uint32_t* first = rows.data() + (size_t)(c - b) * (size_t)n_moduli;
                 if (pairings_vote_rows(first, second, nullptr, (uint64_t)n_moduli) == 0) continue;
                 if (duplicate_mismatches_out) ++*duplicate_mismatches_out;
-                rc = rerun_other_geometry(1, c, c + 1, third); if (rc) return rc;
+                // The tie is broken by the INDEPENDENT implementation, never by the audited one: a deterministic bug
+                // of the fast kernel (a wrong drain, a wrong zero table, a bad new instance) reproduces itself at
+                // any geometry and would out-vote the auditor.  The generic kernel runs once more at another
+                // Gray-bit count; the range stands only if that run sides with the fast row (then the auditor's
+                // first run was the transient fault).  Generic reproducing its own row = the fast row is wrong.
+                rc = rerun_other_geometry(1, c, c + 1, third, &gen); if (rc) return rc;
                 if (pairings_vote_rows(first, second, third, (uint64_t)n_moduli) != 0) return PAIRINGS_ECHECK;
             }
         }

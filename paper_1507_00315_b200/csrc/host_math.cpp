@@ -258,6 +258,37 @@ int pairings_lemma24(int kind, int n) {
     return (e % 2 == 0) ? 1 : 0;
 }
 
+int pairings_mode_chunks(int kind, int n, int chunk_bits, unsigned flags, uint64_t* needed_out) {
+    int rc = check_kind_n(kind, n); if (rc) return rc;
+    rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
+    if (!needed_out) return PAIRINGS_ENULL;
+    if (flags & ~(unsigned)(PAIRINGS_RUN_LEMMA24 | PAIRINGS_RUN_DUPLICATE | PAIRINGS_RUN_AUDIT)) return PAIRINGS_EINVAL_OPTS;
+    uint64_t needed = 1ULL << chunk_bits;
+    int factor = 1;
+    // Lemma 2.4: the most significant chunk bit is x_2, so the x_2 = +1 half of the sum is the chunk
+    // range [0, 2^{C-1}); the other half equals it (factor 2) or cancels it (nothing to evaluate, H = 0).
+    if ((flags & PAIRINGS_RUN_LEMMA24) && chunk_bits >= 1) {
+        if (pairings_lemma24(kind, n) == 1) { needed >>= 1; factor = 2; }
+        else { needed = 0; factor = 0; }
+    }
+    *needed_out = needed;
+    return factor;
+}
+
+int pairings_finish_total(int kind, int n, int chunk_bits, unsigned flags, uint64_t chunks_covered,
+                          const uint32_t* moduli, int n_moduli, uint32_t* total_inout) {
+    uint64_t needed = 0;
+    const int factor = pairings_mode_chunks(kind, n, chunk_bits, flags, &needed); if (factor < 0) return factor;
+    int rc = check_moduli(moduli, n_moduli); if (rc) return rc;
+    if (!total_inout) return PAIRINGS_ENULL;
+    if (chunks_covered > needed) return PAIRINGS_EINVAL_CHUNK;     // more than the mode evaluates: rows of the other half
+    if (chunks_covered < needed) return 0;                         // incomplete: the raw partial sum stays as it is
+    for (int i = 0; i < n_moduli; i++) if (total_inout[i] >= moduli[i]) return PAIRINGS_EINVAL_MODULUS;
+    if (factor == 0) { for (int i = 0; i < n_moduli; i++) total_inout[i] = 0; }
+    else if (factor == 2) { rc = pairings_sum_rows(total_inout, 1, moduli, n_moduli, total_inout); if (rc) return rc; }
+    return 1;
+}
+
 int64_t pairings_partition(int chunk_bits, uint64_t max_chunks, const uint64_t* done, int n_done,
                            uint64_t* out_ranges, int64_t cap_ranges) {
     if (chunk_bits < 0 || chunk_bits > 63 || max_chunks == 0 || n_done < 0) return PAIRINGS_EINVAL_CHUNK;
@@ -472,10 +503,20 @@ int pairings_journal_append(const char* path, int kind, int n, int chunk_bits,
 
 int64_t pairings_journal_merge(const char* const* paths, int n_paths, const char* out_path, int kind, int n, int chunk_bits,
                                const uint32_t* moduli, int n_moduli, uint32_t* total_out, uint64_t* chunks_covered_out) {
+    return pairings_journal_merge_mode(paths, n_paths, out_path, kind, n, chunk_bits, moduli, n_moduli, 0u,
+                                       total_out, chunks_covered_out, nullptr);
+}
+
+int64_t pairings_journal_merge_mode(const char* const* paths, int n_paths, const char* out_path, int kind, int n, int chunk_bits,
+                                    const uint32_t* moduli, int n_moduli, unsigned flags,
+                                    uint32_t* total_out, uint64_t* chunks_covered_out, uint64_t* chunks_needed_out) {
     int rc = check_kind_n(kind, n); if (rc) return rc;
     rc = check_moduli(moduli, n_moduli); if (rc) return rc;
     rc = check_chunks(n, chunk_bits, 0, 0); if (rc) return rc;
     if (!paths || n_paths < 1 || !total_out) return PAIRINGS_ENULL;
+    uint64_t needed = 0;
+    rc = pairings_mode_chunks(kind, n, chunk_bits, flags, &needed); if (rc < 0) return rc;
+    if (chunks_needed_out) *chunks_needed_out = needed;
     for (int i = 0; i < n_moduli; i++) total_out[i] = 0;
     std::vector<JournalLine> all;
     for (int j = 0; j < n_paths; j++) {
@@ -489,6 +530,9 @@ int64_t pairings_journal_merge(const char* const* paths, int n_paths, const char
     uint64_t covered = 0;
     for (size_t i = 0; i < all.size(); i++) {
         if (i && all[i].b < all[i - 1].e) return PAIRINGS_EJOURNAL;   // two journals hold the same chunk: double count
+        // a range outside the half this mode evaluates (a journal of a job without the symmetry, or a mix of both
+        // halves that happens to have the right length) would be doubled into a wrong count
+        if (all[i].e > needed) return PAIRINGS_EJOURNAL;
         covered += all[i].e - all[i].b;
         pairings_sum_rows(all[i].row, 1, moduli, n_moduli, total_out);
     }

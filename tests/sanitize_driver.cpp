@@ -132,6 +132,17 @@ int main(int argc, char** argv) {
         CHECK(pairings_journal_merge(paths, 2, m.c_str(), 1, 12, 6, p, 4, tot, &cov) == 2 && cov == 64 && tot[3] == 8);
         CHECK(pairings_journal_merge(paths, 3, nullptr, 1, 12, 6, p, 4, tot, &cov) == PAIRINGS_EJOURNAL);
         CHECK(pairings_journal_merge(paths, 0, nullptr, 1, 12, 6, p, 4, tot, &cov) == PAIRINGS_ENULL);
+        // the mode of a job: b.txt lies in the x_2 = -1 half, which a Lemma 2.4 job does not evaluate
+        uint64_t need = 0;
+        CHECK(pairings_mode_chunks(1, 12, 6, PAIRINGS_RUN_LEMMA24, &need) == 2 && need == 32);
+        CHECK(pairings_mode_chunks(0, 14, 6, PAIRINGS_RUN_LEMMA24, &need) == 0 && need == 0);
+        CHECK(pairings_mode_chunks(1, 12, 6, 0, nullptr) == PAIRINGS_ENULL);
+        CHECK(pairings_journal_merge_mode(paths, 2, nullptr, 1, 12, 6, p, 4, PAIRINGS_RUN_LEMMA24, tot, &cov, &need) == PAIRINGS_EJOURNAL);
+        CHECK(pairings_journal_merge_mode(paths + 1, 1, nullptr, 1, 12, 6, p, 4, PAIRINGS_RUN_LEMMA24, tot, &cov, &need) == 1 && cov == 32 && need == 32);
+        CHECK(pairings_finish_total(1, 12, 6, PAIRINGS_RUN_LEMMA24, cov, p, 4, tot) == 1 && tot[3] == 2 * row[3] % p[3]);
+        CHECK(pairings_finish_total(1, 12, 6, PAIRINGS_RUN_LEMMA24, 31, p, 4, tot) == 0);
+        CHECK(pairings_finish_total(1, 12, 6, PAIRINGS_RUN_LEMMA24, 33, p, 4, tot) == PAIRINGS_EINVAL_CHUNK);
+        CHECK(pairings_finish_total(1, 12, 6, 0, 64, p, 4, nullptr) == PAIRINGS_ENULL);
         uint32_t x[4] = {1, 2, 3, 4}, y[4] = {1, 2, 3, 5}, z[4] = {7, 7, 7, 7};
         CHECK(pairings_vote_rows(x, x, nullptr, 4) == 0 && pairings_vote_rows(x, y, nullptr, 4) == 3);
         CHECK(pairings_vote_rows(x, y, x, 4) == 0 && pairings_vote_rows(x, y, y, 4) == 1 && pairings_vote_rows(x, y, z, 4) == PAIRINGS_ECHECK);

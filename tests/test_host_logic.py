@@ -305,6 +305,49 @@ def test_journal_merge_puts_rank_journals_together(tmp_path):
         pb.pairings_journal_merge([paths[0], foreign], kind, n, C, moduli)
 
 
+def test_mode_rule_of_lemma24_lives_behind_the_abi(tmp_path):
+    # Lemma 2.4: the x_2 = +1 half is the chunk range [0, 2^(C-1)); equal halves -> factor 2,
+    # cancelling halves -> nothing to evaluate, H = 0.  Pairings exist exactly when the halves are equal.
+    moduli = pb.pairings_default_moduli(4)
+    assert pb.pairings_mode_chunks(1, 12, 6, 0) == (64, 1)
+    assert pb.pairings_mode_chunks(1, 12, 6, pb.RUN_LEMMA24) == (32, 2)            # L(12) exists
+    assert pb.pairings_mode_chunks(1, 12, 0, pb.RUN_LEMMA24) == (1, 1)             # no chunk bit to fix: flag ignored
+    assert pb.pairings_mode_chunks(0, 14, 6, pb.RUN_LEMMA24) == (0, 0)             # S(14) does not exist: halves cancel
+    assert pb.pairings_mode_chunks(0, 13, 6, pb.RUN_LEMMA24 | pb.RUN_AUDIT) == (32, 2)
+    for kind in (0, 1):
+        for n in range(2, 33):
+            exists = n % 4 in ((0, 1) if kind == 0 else (0, 3))
+            assert pb.pairings_mode_chunks(kind, n, 3, pb.RUN_LEMMA24) == ((4, 2) if exists else (0, 0))
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_mode_chunks(1, 12, 6, 64)                                      # unknown flag
+    raw = [5, moduli[1] - 1, 0, 7]
+    assert pb.pairings_finish_total(1, 12, 6, 0, 64, moduli, raw) == (True, raw)
+    assert pb.pairings_finish_total(1, 12, 6, 0, 63, moduli, raw) == (False, raw)
+    assert pb.pairings_finish_total(1, 12, 6, pb.RUN_LEMMA24, 32, moduli, raw) == (True, [10, moduli[1] - 2, 0, 14])
+    assert pb.pairings_finish_total(1, 12, 6, pb.RUN_LEMMA24, 31, moduli, raw) == (False, raw)
+    assert pb.pairings_finish_total(0, 14, 6, pb.RUN_LEMMA24, 0, moduli, raw) == (True, [0, 0, 0, 0])
+    with pytest.raises(pb.PairingsError) as ei:
+        pb.pairings_finish_total(1, 12, 6, pb.RUN_LEMMA24, 33, moduli, raw)        # rows of the other half got in
+    assert ei.value.code == -3
+    # merging in a mode: ranges outside the evaluated half are refused, whatever their total length
+    kind, n, C = 1, 12, 6
+    good, mixed, full = (str(tmp_path / f) for f in ("good.txt", "mixed.txt", "full.txt"))
+    row = [1, 2, 3, 4]
+    pb.pairings_journal_append(good, kind, n, C, moduli, 0, 16, row)
+    pb.pairings_journal_append(good, kind, n, C, moduli, 16, 32, row)
+    assert pb.pairings_journal_merge_mode([good], kind, n, C, moduli, pb.RUN_LEMMA24) == (2, [2, 4, 6, 8], 32, 32)
+    pb.pairings_journal_append(mixed, kind, n, C, moduli, 0, 16, row)              # 16 chunks of each half: length 32
+    pb.pairings_journal_append(mixed, kind, n, C, moduli, 32, 48, row)
+    assert pb.pairings_journal_merge([mixed], kind, n, C, moduli)[2] == 32   # mode-less merge: plain coverage
+    with pytest.raises(pb.PairingsError) as ei:
+        pb.pairings_journal_merge_mode([mixed], kind, n, C, moduli, pb.RUN_LEMMA24)
+    assert ei.value.code == -11
+    pb.pairings_journal_append(full, kind, n, C, moduli, 0, 64, row)               # a job run without the symmetry
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_journal_merge_mode([full], kind, n, C, moduli, pb.RUN_LEMMA24)
+    assert pb.pairings_journal_merge_mode([full], kind, n, C, moduli, 0) == (1, row, 64, 64)
+
+
 def test_duplicate_run_vote_all_outcomes():
     # every job twice, "if there was a mismatch the job was ran a third time to establish a match"
     a, b, c = [1, 2, 3, 4], [1, 2, 3, 5], [9, 9, 9, 9]
@@ -329,6 +372,13 @@ def test_duplicate_run_vote_all_outcomes():
     with pytest.raises(pb.PairingsError) as ei:                   # an evaluation error is passed through
         pb.pairings_duplicate_vote(lambda k: -6 if k == 1 else a, 4)
     assert ei.value.code == -6
+    # an evaluator that raises must not look like two agreeing all-zero attempts (ctypes swallows callback exceptions)
+    def broken(k):
+        raise KeyError("attempt %d failed" % k)
+    with pytest.raises(KeyError):
+        pb.pairings_duplicate_vote(broken, 4)
+    with pytest.raises(ValueError):
+        pb.pairings_duplicate_vote(lambda k: [1, 2, 3], 4)        # a short row would leave a word unfilled
 
 
 def test_run_slice_argument_checks_need_no_gpu():
