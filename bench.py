@@ -21,9 +21,12 @@ its `value` counts the sign vectors ONCE.
 `value`   = terms/s with the rows left in HBM (CUDA events around the kernel launches of a step).
 `e2e`     = terms/s through count_pairings_host (HOST output buffer; allocation, launch, D2H copy
             and synchronise inside the timed region, wall clock).
-`roofline`= SURVEY.md §8(d): `frac` on the fixed yardstick ops/term (W + phi*M, phi measured live) x terms/s
-            against the SM integer-issue peak 148 x 128 lanes x sm_max_mhz; beside it the EXECUTED thread-instructions
-            per term of the profiled kernel (profiles/ncu_metrics.json) and the issue-slot fraction they give.
+`roofline`= `frac` = issue-slot fraction: EXECUTED thread-instructions per term of the profiled kernel
+            (profiles/ncu_metrics.json, ignored when the kernel source changed since the capture) x terms/s measured
+            here, against the SM integer-issue peak 148 x 128 lanes x sm_max_mhz.  Beside it `useful_frac` (the minimum
+            instruction count of the design as built, same rate and peak), `yardstick_frac` (SURVEY.md
+            §8(d)'s fixed model W + phi*M of a scalar kernel: a speed-up over that design, not a utilisation) and
+            `n24`, the S(24) point of the metric with its own fractions and clocks.
 `cpu_baseline` = the CPU oracle (oracle/, as it stands) on the host cores, bounded sample, all cores and 1 core.
 """
 from __future__ import annotations
@@ -75,35 +78,156 @@ def yardstick_ops(kind: int, n: int, n_moduli: int, phi: float):
     return W + phi * M, dict(W=W, M=M, G=G, phi=phi)
 
 
-def ncu_metrics(kind: int, n: int):
-    """The executed-instruction record of the profiled kernel instance (written by
-    `python -m paper_1507_00315_b200.ncu_summary` from an `ncu --set full` capture), or None."""
+KERNEL_SOURCES = {"instances": ["swar_kernel.cuh", "device_common.cuh"], "pt": ["pt_kernel.cu"]}
+
+
+def kernel_source_sha16(which: str) -> str:
+    """sha256 (16 hex digits) over the source files of a profiled kernel — recorded with every ncu capture in
+    profiles/ncu_metrics.json, so that a capture of an older kernel is recognised without git (the GPU box has none)."""
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES[which]:
+        with open(os.path.join(ROOT, "paper_1507_00315_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_record(which: str, key=None):
+    """(record, stale) — the ncu capture of a kernel from profiles/ncu_metrics.json (`which` = "instances" with key
+    "L20", or "pt"); stale = the kernel's source files no longer hash to what the capture recorded.  (None, False)
+    when there is no record."""
     try:
         with open(NCU_METRICS) as f:
-            return json.load(f)["instances"].get("%s%d" % (KIND_NAME[kind], n))
+            doc = json.load(f)
+        rec = doc[which] if key is None else doc[which].get(key)
     except (OSError, ValueError, KeyError):
-        return None
+        return None, False
+    if not rec:
+        return None, False
+    return rec, rec.get("source_sha16") != kernel_source_sha16(which)
+
+
+def swar_plan(kind: int, n: int):
+    """The packed-sum layout and product plan of swar_kernel<kind, n> (csrc/swar_kernel.cuh, Lay::make_plan), restated
+    for the instruction accounting: NR packed registers, E even distances, pair / single factors, G groups with exact
+    products below 2^31 (best fit decreasing), W accumulator words."""
+    N = 2 * n
+    ds = [k if kind == 0 else k + 1 for k in range(1, n + 1)]
+    slots = [d for d in ds if d % 2 == 0] + [d for d in ds if d % 2 == 1]
+    bound = [((N - d) // 2 if d % 2 == 0 else N - d) for d in slots]
+    NR = (n + 3) // 4
+    sb = lambda s: bound[s] if s < n else 0
+
+    def plan(last_as_singles):
+        fac = []                                            # (bound, is_pair)
+        for pp in range(NR // 2):
+            r = 2 * pp
+            for i in range(4):
+                b1, b2 = sb(4 * r + i), sb(4 * (r + 1) + i)
+                if b1 and b2:
+                    fac.append((b1 * b2, True))
+                elif b1:
+                    fac.append((b1, False))
+        if NR % 2 == 1:
+            r = NR - 1
+            for i in range(0, 4, 1 if last_as_singles else 2):
+                b1, b2 = sb(4 * r + i), 0 if last_as_singles else sb(4 * r + i + 1)
+                if b1 and b2:
+                    fac.append((b1 * b2, True))
+                elif b1:
+                    fac.append((b1, False))
+        order = sorted(range(len(fac)), key=lambda f: -fac[f][0])
+        for G in range(1, 9):
+            prod, ok = [1] * G, True
+            for f in order:
+                best = -1
+                for g in range(G):
+                    if prod[g] * fac[f][0] < 1 << 31 and (best < 0 or prod[g] > prod[best]):
+                        best = g
+                if best < 0:
+                    ok = False
+                    break
+                prod[best] *= fac[f][0]
+            if ok:
+                bits = sum(p.bit_length() for p in prod)
+                return dict(G=G, W=(bits + 33 + 31) // 32, nf=len(fac), pairs=sum(1 for f in fac if f[1]),
+                            singles=sum(1 for f in fac if not f[1]))
+        raise ValueError("no grouping")
+
+    a, b = plan(True), plan(False)
+    best = a if a["G"] < b["G"] else b
+    best.update(NR=NR, E=sum(1 for d in ds if d % 2 == 0))
+    return best
+
+
+def useful_instr(kind: int, n: int, phi: float):
+    """Minimum thread-instructions per term of the SWAR design AS BUILT — the method's arithmetic
+    only, no compaction, no loop or address overhead (O(n) additions and multiplications per Gray step):
+      every step        NR packed adds (the n byte sums in NR registers) + 4 E / 32 for the zero test (4 instructions
+                        per even distance and 32-step block: table address, load, OR, predicate extraction)
+      non-zero (x phi)  NR un-bias XORs, 2 per pair factor (operand isolation + IDP.4A) and 1 per single, one 32-bit
+                        multiply per factor into its group, 2 for the sign, wide(G) for the exact multi-word product
+                        (G = 1: 0, 2: 1, 3: 5, 4: 10 IMAD.WIDE / digit splits; G >= 5: G(G-1)/2 + G + W + 2),
+                        W add-with-carry into the accumulator."""
+    pl = swar_plan(kind, n)
+    G, W = pl["G"], pl["W"]
+    wide = {1: 0, 2: 1, 3: 5, 4: 10}.get(G, G * (G - 1) // 2 + G + W + 2)
+    per_step = pl["NR"] + 4.0 * pl["E"] / 32
+    per_nonzero = pl["NR"] + 2 * pl["pairs"] + pl["singles"] + pl["nf"] + 2 + wide + W
+    return per_step + phi * per_nonzero, dict(plan=pl, per_step=per_step, per_nonzero_term=per_nonzero, phi=phi)
 
 
 def roofline_object(kind, n, n_moduli, phi, terms_per_launch, kernel_s, peak_mhz):
-    """SURVEY §8(d)'s three numbers: terms/s (in the line), the model fraction on the fixed yardstick (`frac`), and
-    the executed thread-instructions per term with the issue-slot fraction they give."""
+    """`frac` = executed thread-instructions (ncu capture of this kernel instance) x terms/s (measured here) / issue
+    peak; `useful_frac` = the design's minimum instruction count at the same rate; `yardstick_frac` = SURVEY §8(d)'s
+    model of a scalar kernel (> 1 here: the kernel needs fewer instructions than that model, it skips no work)."""
     ops, ys = yardstick_ops(kind, n, n_moduli, phi)
     peak = SM_COUNT * LANES_PER_SM_CLK * peak_mhz * 1e6
     rate = terms_per_launch / kernel_s
-    achieved = ops * rate
-    r = dict(bound="alu", achieved=achieved / 1e12, peak=peak / 1e12, unit="Tinstr/s", frac=achieved / peak, traffic=None,
+    useful, ud = useful_instr(kind, n, phi)
+    r = dict(bound="alu", achieved=None, peak=peak / 1e12, unit="Tinstr/s", frac=None, traffic=None,
              peak_source="formula: 148 SM x 128 lanes/clk x %.0f MHz (clocks.max.sm); MEASURED_PEAKS.json has no integer figure" % peak_mhz,
-             ops_per_term=ops, yardstick=ys, kernel_ms=kernel_s * 1e3, terms_per_launch=terms_per_launch,
-             frac_note="frac is on the fixed yardstick of SURVEY.md §8(d) (3n+3 scalar ops per step, per-term Montgomery chains); this "
-                       "kernel needs fewer instructions than that (packed sums, table-driven zero test, residues once per thread), so "
-                       "frac > 1; issue_frac = executed instructions x terms/s / peak is the utilisation figure")
-    m = ncu_metrics(kind, n)
-    if m:
-        r.update(executed_instr_per_term=m["instr_per_term"], issue_frac=m["instr_per_term"] * rate / peak,
-                 issue_active_pct=m["issue_active_pct"], ncu_source=m.get("source"), ncu_commit=m.get("commit"),
-                 traffic=m.get("dram_bytes_per_launch"))
+             kernel_ms=kernel_s * 1e3, terms_per_launch=terms_per_launch, terms_per_s=rate,
+             useful_instr_per_term=useful, useful_frac=useful * rate / peak, useful_model=ud,
+             ops_per_term=ops, yardstick=ys, yardstick_frac=ops * rate / peak,
+             frac_note="frac = executed thread-instructions per term (ncu) x terms/s (CUDA events, this run) / peak: issue slots busy. "
+                       "useful_frac = minimum instruction count of the design as built (DESIGN.md 4.3) at the same rate: issue slots "
+                       "doing Godfrey arithmetic. yardstick_frac = SURVEY 8(d)'s fixed model of a scalar per-term-Montgomery kernel, "
+                       "> 1 because this kernel needs fewer instructions than that model (packed sums, table-driven zero test, "
+                       "residues once per thread); the count is reconstructed and checked in every run")
+    m, stale = ncu_record("instances", "%s%d" % (KIND_NAME[kind], n))
+    if m and not stale:
+        r.update(executed_instr_per_term=m["instr_per_term"], achieved=m["instr_per_term"] * rate / 1e12,
+                 frac=m["instr_per_term"] * rate / peak, issue_active_pct=m["issue_active_pct"], ncu_source=m.get("source"),
+                 ncu_commit=m.get("commit"), ncu_source_sha16=m.get("source_sha16"), traffic=m.get("dram_bytes_per_launch"))
+    elif m:
+        r.update(ncu_stale=True, ncu_commit=m.get("commit"),
+                 ncu_note="the kernel source changed since the ncu capture in profiles/ncu_metrics.json: no executed-instruction "
+                          "figure is claimed for this build (frac = null); useful_frac and yardstick_frac need no capture")
     return r
+
+
+def exchange_sums(dist, total, moduli, world, duplicate, device, sum_rows):
+    """The ONE exchange of the N > 1 path ("simply put the result together at the end"): every rank's
+    residue sums are gathered and added modulo the primes (disjoint ranges), or compared (duplicate-run check,
+    PAPER.md:99).  `dist` = torch.distributed with an initialised default group (NCCL on GPUs, gloo in the CPU tests);
+    `sum_rows(rows, moduli)` = pairings_sum_rows.  Returns the job's residue sums on every rank."""
+    import torch
+    t = torch.tensor(total, dtype=torch.int64, device=device)
+    gathered = [torch.zeros_like(t) for _ in range(world)]
+    dist.all_gather(gathered, t)
+    if duplicate:                                    # every rank counted everything: the copies must agree
+        assert all(g.tolist() == list(total) for g in gathered), "ranks disagree (PAPER.md:99 duplicate-run check)"
+        return list(total)
+    return sum_rows([g.tolist() for g in gathered], moduli)
+
+
+def max_over_ranks(dist, x: float, device) -> float:
+    """A time is the slowest rank's."""
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
 
 
 def host_threads() -> int:
@@ -309,8 +433,7 @@ def run_gpu(args):
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")      # > 126 MB L2
 
     def launch_opts(nonzero_ptr=None):
-        o = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=args.gray_bits, block_threads=args.block_threads,
-                          blocks_per_chunk=args.blocks_per_chunk)
+        o = pb.LaunchOpts(variant=pb.VARIANT_AUTO, gray_bits=0, block_threads=0, blocks_per_chunk=0)   # library defaults
         if nonzero_ptr is not None:
             o.nonzero_terms = nonzero_ptr
         return o
@@ -331,13 +454,7 @@ def run_gpu(args):
         flat = (ctypes.c_uint32 * (rows * m)).from_address(rows_tensor.data_ptr())
         total = pb.pairings_sum_rows(flat, moduli)
         if dist is not None:
-            t = torch.tensor(total, dtype=torch.int64, device="cuda")
-            gathered = [torch.zeros_like(t) for _ in range(world)]
-            dist.all_gather(gathered, t)
-            if duplicate:                                # every rank counted everything: the copies must agree
-                assert all(g.tolist() == total for g in gathered), "ranks disagree (PAPER.md:99 duplicate-run check)"
-            else:
-                total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
+            total = exchange_sums(dist, total, moduli, world, duplicate, "cuda", pb.pairings_sum_rows)
         if rank == 0 and not args.profile_chunks:
             D, S = pb.pairings_reconstruct(kind, n, moduli, total)
             assert S == L20_IDENTIFIED and D == 2 * S, ("L(20) mismatch", D, S)
@@ -378,9 +495,7 @@ def run_gpu(args):
     dev_ms = sum(a.elapsed_time(b) for a, b in evs)
     rank_kernel_s = dev_ms * 1e-3 / args.steps            # this rank's kernel
     if dist is not None:
-        t = torch.tensor([dev_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dev_ms = float(t.item())
+        dev_ms = max_over_ranks(dist, dev_ms, "cuda")
     launches = (warm + 1 + args.steps) * world  # one kernel launch per pass and rank (grid = chunks of the rank)
     value = terms_job * args.steps / (dev_ms * 1e-3)
 
@@ -396,9 +511,7 @@ def run_gpu(args):
     e2e_s = time.perf_counter() - t0
     clocks_e2e = sampler.window(t0, t0 + e2e_s)
     if dist is not None:
-        t = torch.tensor([e2e_s], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_s = float(t.item())
+        e2e_s = max_over_ranks(dist, e2e_s, "cuda")
     e2e_value = terms_job * args.steps / e2e_s
     launches += (2 + args.steps) * world
 
@@ -434,9 +547,8 @@ def run_gpu(args):
                 best = max(best, cnt / (e0.elapsed_time(e1) * 1e-3))
             cal[name] = best / 1e12
         roofline["calibration_Tinstr_per_s"] = cal
-        roofline["frac_of_best_calibration"] = roofline["achieved"] / max(cal.values())
-        if "issue_frac" in roofline:
-            roofline["issue_frac_of_best_calibration"] = roofline["issue_frac"] * roofline["peak"] / max(cal.values())
+        if roofline["achieved"] is not None:       # against the best measured instruction mix instead of the formula peak
+            roofline["frac_of_best_calibration"] = roofline["achieved"] / max(cal.values())
 
         # secondary point of the metric: S(24) on the seeded 1/64 subset (BASELINE.json configs[4])
         n24 = None
@@ -474,6 +586,13 @@ def run_gpu(args):
                                          pb.pairings_query_geometry(k2, n2, C2, WL24["run_len"], opts))),
                        clocks=sampler.window(t0, t1), projected_full_run_s=(1 << 47) / (terms24 / t24),
                        roofline=roofline_object(k2, n2, m2, phi24, terms24 // len(starts), t24 / len(starts), peak_mhz))
+            # the n = 24 half of BASELINE.json's metric, inside the objects the driver keeps
+            r24 = n24["roofline"]
+            roofline["n24"] = dict(workload=n24["workload"], value=n24["value"], unit="terms/s", seconds=t24, terms=terms24,
+                                   frac=r24["frac"], useful_frac=r24["useful_frac"], yardstick_frac=r24["yardstick_frac"],
+                                   executed_instr_per_term=r24.get("executed_instr_per_term"),
+                                   useful_instr_per_term=r24["useful_instr_per_term"], phi=phi24, clocks=n24["clocks"],
+                                   projected_full_run_s=n24["projected_full_run_s"], ncu_stale=r24.get("ncu_stale", False))
 
         # the other BASELINE.json configs (parity-test cases; timed here for SURVEY §8(d)'s per-config table)
         other = None
@@ -502,7 +621,9 @@ def run_gpu(args):
                 ops2, ys2 = yardstick_ops(k2, n2, m2, phi2)
                 entry = dict(config="%s(%d)" % (KIND_NAME[k2], n2), chunk_bits=C2, n_moduli=m2, launches_timed=reps,
                              seconds_per_count=sec, value=terms2 / sec, unit="terms/s", phi=phi2, ops_per_term=ops2,
-                             roofline_frac=ops2 * terms2 / sec / peak, identified=S2,
+                             yardstick_frac=ops2 * terms2 / sec / peak,
+                             useful_frac=useful_instr(k2, n2, phi2)[0] * terms2 / sec / peak if pb.pairings_has_swar(k2, n2) else None,
+                             identified=S2,
                              geometry=dict(zip(("variant", "gray_bits", "block_threads", "blocks_per_chunk"),
                                                pb.pairings_query_geometry(k2, n2, C2, rows2, opts))))
                 if reps >= 20:
@@ -524,12 +645,14 @@ def run_gpu(args):
                     launches += 2 * reps
                     flat2 = (ctypes.c_uint32 * (rows2 * m2)).from_buffer_copy(out2.cpu().numpy().tobytes())
                     assert pb.pairings_reconstruct(k2, n2, mod2, pb.pairings_sum_rows(flat2, mod2))[1] == want
+                m2rec, stale2 = ncu_record("instances", "%s%d" % (KIND_NAME[k2], n2))
+                if m2rec and not stale2:
+                    entry.update(executed_instr_per_term=m2rec["instr_per_term"], frac=m2rec["instr_per_term"] * terms2 / sec / peak)
                 other.append(entry)
 
         # second workload: the approximate counter, S(12) with the ladder of Table 6
         ptres = None
         if not args.no_pt and extras:
-            import math
             R, T, burn = 1 << 17, 1 << 11, 0                      # throughput run (too short per replica for an estimate)
             Mlev = len(PT_BETAS)
             h = torch.zeros((Mlev, 25), dtype=torch.int64, device="cuda")
@@ -551,7 +674,7 @@ def run_gpu(args):
             est_s = time.perf_counter() - t0
             launches += 3
             ratios, logz = pb.pairings_pt_estimate(0, 12, PT_BETAS, h.cpu().tolist())
-            est = math.exp(logz) / 2
+            est = pb.pairings_pt_counts(12, logz)[1]
             moves_s = R * T * Mlev / sec
             ptres = dict(workload="approximate count of S(12), 12 levels (Table 6 ladder, PAPER.md:327-342)",
                          replicas=R, iterations=T, seconds=sec, metropolis_moves_per_s=moves_s,
@@ -560,17 +683,18 @@ def run_gpu(args):
                                        s12_estimate=est, exact=227968, rel_error=est / 227968 - 1))
             if ptres["cpu_oracle"]:
                 ptres["gpu_over_cpu_oracle"] = moves_s / ptres["cpu_oracle"]["value"]
-            try:                                        # yardstick: executed instruction slots per move x moves/s against the issue peak
-                with open(NCU_METRICS) as f:
-                    pm = json.load(f)["pt"]
+            pm, pstale = ncu_record("pt")               # executed instruction slots per move x moves/s against the issue peak
+            if pm and not pstale:
                 ptres["roofline"] = dict(bound="alu", thread_instr_slots_per_move=pm["thread_instr_slots_per_move"],
-                                         issue_frac=pm["thread_instr_slots_per_move"] * moves_s / peak, issue_active_pct=pm["issue_active_pct"],
+                                         frac=pm["thread_instr_slots_per_move"] * moves_s / peak, issue_active_pct=pm["issue_active_pct"],
                                          active_threads_per_warp_instr=pm["active_threads_per_warp_instr"], ncu_source=pm["source"],
+                                         ncu_commit=pm.get("commit"),
                                          work_model="per move: one 64-bit SplitMix draw for colour and position (+ one for the acceptance when dE > 0), "
                                                     "5 shared loads (old position, 4 bins), 5 shared stores when accepted; per level and iteration one "
                                                     "histogram atomic and one exchange test (+ draw when dE > 0)")
-            except (OSError, ValueError, KeyError):
-                pass
+            elif pm:
+                ptres["roofline"] = dict(ncu_stale=True, ncu_commit=pm.get("commit"),
+                                         ncu_note="pt_kernel.cu changed since the ncu capture: no issue fraction is claimed for this build")
 
         cpu = cpu_baseline(kind, n) if not args.no_cpu and not args.profile_chunks else None
         par = ("every rank the whole pass x%d, residue sums cross-checked (PAPER.md:99); each sign vector counted once" if duplicate
@@ -585,7 +709,9 @@ def run_gpu(args):
                                 sm_count=torch.cuda.get_device_properties(local).multi_processor_count,
                                 l2="flushed between steps (256 MiB fill); the kernel reads no global memory but its 24 KB zero-step tables",
                                 result_check="L(20) = 2,636,337,861,200 reconstructed every run (PAPER.md:380)",
-                                library=pb.pairings_build_info()),
+                                library=pb.pairings_build_info(),
+                                n24=None if n24 is None else dict(workload=n24["workload"], terms_per_s=n24["value"], seconds=n24["seconds"],
+                                                                  sm_mhz=n24["clocks"].get("sm_mhz"), reasons=n24["clocks"].get("reasons"))),
                     clocks=clocks,
                     e2e=dict(value=e2e_value, unit="terms/s", h2d_bytes_per_step=(4 * m + 8 * 5) * world,
                              d2h_bytes_per_step=rows * m * 4 * world, seconds_per_step=e2e_s / args.steps,
@@ -636,19 +762,39 @@ def _free_port():
     return p
 
 
-def spawn_ranks(n: int) -> int:
+def spawn_ranks(n: int, poll_s: float = 0.2, command=None) -> int:
     """Starts n copies of this command line, one rank each (rank r -> cuda:r), and waits for them.  Rank 0's stdout is
-    this process's stdout (the JSON line); NCCL's own logging is left as the environment has it."""
+    this process's stdout (the JSON line); NCCL's own logging is left as the environment has it.  The library is built
+    once here, before the ranks start (they would race to write the same objects on a fresh checkout).  The ranks are
+    polled: as soon as one exits non-zero the others — which would wait for it in the NCCL rendezvous or a barrier
+    for ever — are terminated and that exit code is returned."""
+    if command is None:
+        from paper_1507_00315_b200 import build as pbuild
+        pbuild.build()
+        command = [sys.executable, os.path.abspath(__file__)] + sys.argv[1:]
     port = os.environ.get("MASTER_PORT") or str(_free_port())
     procs = []
     for r in range(n):
         env = dict(os.environ, RANK=str(r), LOCAL_RANK=str(r), WORLD_SIZE=str(n), MASTER_ADDR="127.0.0.1", MASTER_PORT=port,
                    PAIRINGS_BENCH_SPAWNED="1")
-        procs.append(subprocess.Popen([sys.executable, os.path.abspath(__file__)] + sys.argv[1:], env=env,
-                                      stdout=None if r == 0 else subprocess.DEVNULL))
-    rc = 0
-    for p in procs:
-        rc = max(rc, abs(p.wait()))
+        procs.append(subprocess.Popen(command, env=env, stdout=None if r == 0 else subprocess.DEVNULL))
+    rc, live = 0, list(procs)
+    while live and rc == 0:
+        time.sleep(poll_s)
+        for p in list(live):
+            code = p.poll()
+            if code is None:
+                continue
+            live.remove(p)
+            if code != 0:
+                rc = abs(code) or 1
+    for p in live:                                   # a rank failed: the rest cannot finish
+        p.terminate()
+    for p in live:
+        try:
+            p.wait(timeout=10)
+        except subprocess.TimeoutExpired:
+            p.kill()
     return rc
 
 
@@ -667,11 +813,9 @@ def main():
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
     ap.add_argument("--no-pt", action="store_true", help="skip the approximate-counter (parallel tempering) measurement")
     ap.add_argument("--no-configs", action="store_true", help="skip the timing of the other BASELINE configs")
-    ap.add_argument("--gray-bits", type=int, default=0, help="sweep aid: pin pairings_launch_opts.gray_bits (0 = library default)")
-    ap.add_argument("--block-threads", type=int, default=0, help="sweep aid: pin block_threads (0 = library default)")
-    ap.add_argument("--blocks-per-chunk", type=int, default=0, help="sweep aid: pin blocks_per_chunk (0 = library default)")
     ap.add_argument("--profile-chunks", type=int, default=0,
-                    help="profiling aid: only the first N chunks per step (short launches for ncu); the line is marked, not a bench value")
+                    help="only the first N chunks per step: the short launches the ncu commands in profiles/ capture; the line is "
+                         "marked profile_only, it is not a bench value")
     args = ap.parse_args()
     if args.gpus < 1:
         ap.error("--gpus must be >= 1")

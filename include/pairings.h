@@ -391,6 +391,11 @@ int pairings_pt_ladder(int kind, int n, double target_exchange, uint64_t pilot_r
 int pairings_pt_estimate(int kind, int n, const double* betas, int n_levels, const uint64_t* hist_host,
                          double* ratios_out, double* log_distinct_out);
 
+/* Host: the two counting conventions from the estimate's logarithm (reflections distinct vs identified —
+ * "the two different ways to count differ by exactly a factor of two" for n > 1; Table 6's caption and Tables 7/8 print
+ * the identified count).  *distinct_out = exp(log_distinct), *identified_out = half of it (n > 1). */
+int pairings_pt_counts(int n, double log_distinct, double* distinct_out, double* identified_out);
+
 const char* pairings_strerror(int code);
 
 /* Library build string: version, CUDA arch, compiled SWAR specialisations. */

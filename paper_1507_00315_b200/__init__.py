@@ -14,6 +14,6 @@ from .api import (  # noqa: F401
     pairings_mode_chunks, pairings_finish_total, pairings_vote_rows, pairings_duplicate_vote,
     default_chunk_bits, default_chunks_per_call,
     pairings_reconstruct, pairings_crt_signed, pairings_strerror, pairings_build_info,
-    pairings_pt_run, pairings_pt_run_noalloc, pairings_pt_estimate, pairings_pt_ladder,
+    pairings_pt_run, pairings_pt_run_noalloc, pairings_pt_estimate, pairings_pt_counts, pairings_pt_ladder,
     count, approx_count,
 )

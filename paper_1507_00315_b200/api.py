@@ -82,6 +82,7 @@ def lib():
         "pairings_pt_run": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64, u64, u64, u64, u64, vp, vp, vp, vp]),
         "pairings_pt_run_noalloc": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64, u64, u64, u64, u64, vp, vp, vp, vp]),
         "pairings_pt_ladder": (i, [i, i, ctypes.c_double, u64, u64, u64, ctypes.POINTER(ctypes.c_double), i, vp]),
+        "pairings_pt_counts": (i, [i, ctypes.c_double, ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
         "pairings_pt_estimate": (i, [i, i, ctypes.POINTER(ctypes.c_double), i, u64p, ctypes.POINTER(ctypes.c_double),
                                      ctypes.POINTER(ctypes.c_double)]),
         "pairings_strerror": (cp, [i]),
@@ -402,12 +403,18 @@ def pairings_pt_estimate(kind, n, betas, hist):
     return [float(v) for v in r], float(lz.value)
 
 
+def pairings_pt_counts(n: int, log_distinct: float):
+    """(distinct, identified) estimates from pairings_pt_estimate's logarithm (Table 6 caption)."""
+    d, s_ = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(lib().pairings_pt_counts(n, log_distinct, ctypes.byref(d), ctypes.byref(s_)), "pairings_pt_counts")
+    return float(d.value), float(s_.value)
+
+
 def approx_count(kind: int, n: int, replicas: int = 1 << 12, iterations: int = 1 << 16, burn_in: Optional[int] = None,
                  seed: int = 150700315, betas=None, target_exchange: float = 0.55, device_alloc=None):
     """Convenience: the approximate counter end to end (§3) — ladder (unless given), one pairings_pt_run,
     estimate.  Needs torch for the device counters unless `device_alloc(n_uint64) -> (ptr, read)` is given.
     Returns dict(identified, distinct, betas, ratios, moves, swaps, samples)."""
-    import math
     import torch
     if betas is None:
         betas = pairings_pt_ladder(kind, n, target_exchange, 256, 1 << (14 if n <= 16 else 18), seed ^ 0x5bd1e995)
@@ -426,7 +433,8 @@ def approx_count(kind: int, n: int, replicas: int = 1 << 12, iterations: int = 1
     torch.cuda.synchronize()
     h = hist.cpu().tolist()
     ratios, logz = pairings_pt_estimate(kind, n, betas, h)
-    return dict(distinct=math.exp(logz), identified=math.exp(logz) / 2, betas=betas, ratios=ratios,
+    distinct, identified = pairings_pt_counts(n, logz)
+    return dict(distinct=distinct, identified=identified, betas=betas, ratios=ratios,
                 moves=mv.cpu().tolist(), swaps=sw.cpu().tolist(), samples=replicas * (iterations - burn_in))
 
 

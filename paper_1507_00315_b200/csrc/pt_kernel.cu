@@ -408,4 +408,13 @@ int pairings_pt_estimate(int kind, int n, const double* betas, int n_levels, con
     return PAIRINGS_OK;
 }
 
+int pairings_pt_counts(int n, double log_distinct, double* distinct_out, double* identified_out) {
+    if (n < 2 || n > 32) return PAIRINGS_EINVAL_N;
+    if (!distinct_out || !identified_out) return PAIRINGS_ENULL;
+    if (!std::isfinite(log_distinct)) return PAIRINGS_ERANGE;
+    *distinct_out = std::exp(log_distinct);
+    *identified_out = 0.5 * *distinct_out;          // n > 1: a pairing is never its own reflection
+    return PAIRINGS_OK;
+}
+
 }  // extern "C"

@@ -488,12 +488,6 @@ __device__ __forceinline__ void drain_entry(uint32_t addr, uint32_t k1, uint32_t
             lds_v4(addr + pl * L::PLANE_BYTES, e[4 * pl], e[4 * pl + 1], e[4 * pl + 2], e[4 * pl + 3]);
         });
     }
-#ifdef PAIRINGS_EXP_NODRAIN
-    { uint32_t x = 0;
-#pragma unroll
-      for (int i = 0; i < NR; i++) x ^= e[i];
-      acc[0] += x; return; }
-#endif
     uint32_t w[NR];
     static_for<0, NR>([&](auto rc) {                                              // bytes -> two's complement Q
         PAIRINGS_IC(r, rc);
@@ -671,10 +665,6 @@ struct Walker {
     template <int S>
     __device__ __forceinline__ void push_if_nonzero() {
         constexpr uint32_t bit = 1u << S;
-#ifdef PAIRINGS_EXP_NOSTORE
-        if constexpr (S % QUAD != QUAD - 1) add16_clr(slot, ZM, bit);
-        return;
-#endif
         // entry words: Q[0..NR); plane p holds words 4p..4p+3 (predicated vector stores, no branch)
         if constexpr (L::COMPACT1) {
             sts_v4_clr(slot, Q[0], Q[1], Q[2], Q[3], ZM, bit);

@@ -292,6 +292,18 @@ def test_full_totals_match_the_paper(kind, n, C, paper_counts):
     assert pb.count(kind, n, lemma24=True) == (D, Sid)
 
 
+@pytest.mark.parametrize("kind,n", [(S, 24), (L, 24)])
+def test_full_n24_counts_match_the_paper(kind, n, paper_counts, paper_distinct):
+    # BASELINE.json configs[4]: "full run matched against the paper's printed S(24) if within budget" — it is: 2^46 sign
+    # vectors (symmetry 3: the x_2 = +1 half of the 2^47) in about 70 s.  S(24) = 102,388,058,845,620,672 (PAPER.md:9,
+    # Table 4 :103), A004075(24) = 204,776,117,691,241,344 (:109); L(24) = 46,845,158,056,515,936 (Table 8, :382).
+    D, Sid = pb.count(kind, n, lemma24=True)
+    assert Sid == paper_counts[(kind, n)] and D == 2 * Sid
+    assert Sid == (102388058845620672 if kind == S else 46845158056515936)
+    if (kind, n) in paper_distinct:
+        assert D == paper_distinct[(kind, n)]
+
+
 @pytest.mark.parametrize("kind,n,C", [(L, 12, 6), (S, 13, 8), (L, 8, 3), (S, 16, 10)])
 def test_duplicate_run_mode_and_tight_moduli(kind, n, C, paper_counts):
     # §8(f) NEXT #3 (every job twice, third run on mismatch) and NEXT #2 (tight prime budget)
@@ -306,7 +318,11 @@ def test_duplicate_run_mode_and_tight_moduli(kind, n, C, paper_counts):
 
 
 # ---- the remaining exact values of Tables 7/8 the SWAR kernel is compiled for
-@pytest.mark.parametrize("kind,n,C,count,pieces", [(S, 9, 4, 16, 1), (L, 15, 12, 8, 1), (S, 17, 16, 8, 1), (L, 19, 20, 8, 1),
+# (L(7) at C = 3 is the only geometry that launches swar_kernel<1,7>; S(8), L(8), S(20) were checked through totals only,
+# L(24) not at all before round 3)
+@pytest.mark.parametrize("kind,n,C,count,pieces", [(L, 7, 3, 8, 1), (L, 7, 0, 1, 1), (S, 8, 4, 16, 1), (L, 8, 4, 16, 1),
+                                                   (S, 20, 16, 8, 1), (L, 24, 20, 3, 16),
+                                                   (S, 9, 4, 16, 1), (L, 15, 12, 8, 1), (S, 17, 16, 8, 1), (L, 19, 20, 8, 1),
                                                    (L, 23, 22, 3, 16), (S, 25, 26, 3, 16), (L, 27, 30, 3, 16),
                                                    (S, 28, 32, 3, 16), (L, 28, 32, 3, 16), (S, 29, 34, 3, 16)])
 def test_more_instances_sampled_chunks_match_oracle(kind, n, C, count, pieces):

@@ -348,6 +348,17 @@ def test_mode_rule_of_lemma24_lives_behind_the_abi(tmp_path):
     assert pb.pairings_journal_merge_mode([full], kind, n, C, moduli, 0) == (1, row, 64, 64)
 
 
+def test_pt_counts_conventions():
+    # the conventions differ by exactly a factor of two (n > 1); Table 6 caption prints the identified count
+    import math
+    d, s_ = pb.pairings_pt_counts(12, math.log(455936.0))
+    assert abs(d - 455936.0) < 1e-6 and s_ == d / 2                 # S(12) = 227,968
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_pt_counts(12, float("inf"))
+    with pytest.raises(pb.PairingsError):
+        pb.pairings_pt_counts(1, 0.0)
+
+
 def test_duplicate_run_vote_all_outcomes():
     # every job twice, "if there was a mismatch the job was ran a third time to establish a match"
     a, b, c = [1, 2, 3, 4], [1, 2, 3, 5], [9, 9, 9, 9]

@@ -30,30 +30,39 @@ def _worker(rank, world, port, kind, n, C, q):
     b, e = pb.pairings_rank_range(C, rank, world)
     rows = [oracle.chunk(kind, n, C, c, moduli)[2] for c in range(b, e)]
     mine = pb.pairings_sum_rows(rows, moduli)
-    t = torch.tensor(mine, dtype=torch.int64)
-    gathered = [torch.zeros_like(t) for _ in range(world)]
-    dist.all_gather(gathered, t)
-    total = pb.pairings_sum_rows([g.tolist() for g in gathered], moduli)
+    import bench                                   # bench.py's OWN exchange and time reduction, on gloo instead of NCCL
+    total = bench.exchange_sums(dist, mine, moduli, world, False, "cpu", pb.pairings_sum_rows)
+    # duplicate-run mode: every rank holds the whole sum, the copies are compared
+    same = bench.exchange_sums(dist, total, moduli, world, True, "cpu", pb.pairings_sum_rows)
+    slowest = bench.max_over_ranks(dist, 10.0 + rank, "cpu")
+    disagree = False
+    try:                                           # a rank with another sum must be noticed by every rank
+        bench.exchange_sums(dist, [(v + (rank == world - 1)) % p for v, p in zip(total, moduli)], moduli, world, True, "cpu",
+                            pb.pairings_sum_rows)
+    except AssertionError:
+        disagree = True
     if rank == 0:
-        q.put((b, e, pb.pairings_reconstruct(kind, n, moduli, total)))
+        q.put((b, e, pb.pairings_reconstruct(kind, n, moduli, total), same == total, slowest, disagree))
     dist.barrier()
     dist.destroy_process_group()
 
 
-@pytest.mark.parametrize("kind,n,C,want", [(1, 8, 4, (300, 150)), (0, 9, 5, (2656, 1328)), (0, 7, 3, (0, 0))])
-def test_two_ranks_disjoint_ranges_then_crt(kind, n, C, want):
+@pytest.mark.parametrize("kind,n,C,world,want", [(1, 8, 4, 2, (300, 150)), (0, 9, 5, 2, (2656, 1328)), (0, 7, 3, 2, (0, 0)),
+                                                 (1, 8, 4, 3, (300, 150))])
+def test_ranks_take_disjoint_ranges_then_bench_exchange_then_crt(kind, n, C, world, want):
     from paper_1507_00315_b200 import build as pbuild
     pbuild.build()
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    procs = [ctx.Process(target=_worker, args=(r, 2, port, kind, n, C, q)) for r in range(2)]
+    procs = [ctx.Process(target=_worker, args=(r, world, port, kind, n, C, q)) for r in range(world)]
     [p.start() for p in procs]
-    b, e, got = q.get(timeout=120)
+    b, e, got, same, slowest, disagree = q.get(timeout=180)
     [p.join(timeout=120) for p in procs]
     assert all(p.exitcode == 0 for p in procs)
-    assert (b, e) == (0, 1 << (C - 1))
+    assert (b, e) == (0, (1 << C) // world)
     assert got == want          # L(8)=150, S(9)=1,328, S(7): no pairing
+    assert same and disagree and slowest == 10.0 + world - 1
 
 
 def test_cli_merges_two_rank_journals_of_L12(tmp_path, capsys):
