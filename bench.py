@@ -307,9 +307,9 @@ def run_reference(args):
     line = dict(impl="reference", metric="godfrey_sign_vector_terms_per_s", value=value, unit="terms/s",
                 n_gpus=args.gpus, steps=steps, warmup=warm, ms_per_step=1e3 * t_total / steps,
                 higher_is_better=True, scaling="strong", vs_baseline=None, dtype="int32", data="synthetic",
-                config=dict(workload=WORKLOAD, kind="langford", n=n, chunk_bits=WL["chunk_bits"], n_moduli=WL["n_moduli"],
-                            sample="each step is a bounded sample of the workload: " + sample),
-                cpu_baseline=dict(value=value, unit="terms/s", cores=threads, kind="oracle", sample=sample),
+                config=dict(workload=WORKLOAD, kind="langford", n=n, chunk_bits=WL["chunk_bits"], n_moduli=WL["n_moduli"]),
+                cpu_baseline=dict(value=value, unit="terms/s", cores=threads, kind="oracle",
+                                  sample="each step is a bounded sample of the workload: " + sample),
                 e2e=dict(value=value, unit="terms/s", h2d_bytes_per_step=0, d2h_bytes_per_step=0),
                 gpu_launches=0)
     print(json.dumps(line))
