@@ -85,3 +85,24 @@ def test_noalloc_refuses_what_does_not_fit_its_table():
     with pytest.raises(pb.PairingsError) as bad:
         pb.pairings_pt_run_noalloc(L, 32, [0.5, 1.0], 0, 1, 10, 0, 1, 0, 0, 0)    # betas[0] must be 0, as in pairings_pt_run
     assert bad.value.code == -10
+
+
+def test_noalloc_entry_point_names_no_allocating_call():
+    """A source-level guard for the promise in the header: between its opening brace and the next top-level function,
+    pairings_pt_run_noalloc (and the address look-up it uses) must not mention cudaMalloc*, cudaFree*, a memory pool or
+    a std::vector, and the look-up must go through cudaGetSymbolAddress with its return code checked."""
+    import os
+    import re
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    src = open(os.path.join(root, "paper_1507_00315_b200", "csrc", "pt_kernel.cu")).read()
+    src = re.sub(r"//[^\n]*", "", src)                                        # comments may name what is avoided
+    body = src[src.index("int pairings_pt_run_noalloc("):]
+    body = body[:body.index("\nint pairings_pt_ladder(")]
+    lookup = src[src.index("static int pt_static_address("):]
+    lookup = lookup[:lookup.index("\n}\n") + 3]
+    for text in (body, lookup):
+        for banned in ("cudaMalloc", "cudaFree", "cudaMemPool", "cudaHostAlloc", "std::vector", "new ", "malloc("):
+            assert banned not in text, banned
+    assert "pt_static_address(&table)" in body and "PAIRINGS_ETOOBIG" in body
+    assert re.search(r"cudaGetSymbolAddress\(&ptr, pt_static_thr\)", lookup) and "e != cudaSuccess" in lookup
+    assert re.search(r"static __device__ __align__\(256\) unsigned long long pt_static_thr\[PAIRINGS_PT_STATIC_WORDS\]", src)
